@@ -1,0 +1,145 @@
+/*
+ * qft.h -- C ABI of the B200-native QFT / AQFT executor (libqft.so).
+ *
+ * The library executes the n-qubit QFT circuit of arxiv/paper_2606_18981
+ * ("Not Your Usual FFT: QFT -> FFT via Classical Quantum-Circuit Simulation")
+ * in place on a complex64 state vector of N = 2^n amplitudes that lives in the
+ * memory of one B200:
+ *
+ *     for t = n-1 .. 0:   H(q_t);  CR_{d+1}(q_{t-d} -> q_t), d = 1 .. min(k, t)
+ *     then the bit-reversal swaps SWAP(q_i, q_{n-1-i}), i < floor(n/2)
+ *
+ * (Fig. 1, PAPER.md:116 for the range-k truncation, PAPER.md:137
+ * for the swaps), so that for k >= n-1 the result is the DFT of the input,
+ *
+ *     state[K] <- c * sum_j state[j] * exp(sign * 2 pi i * j K / N),
+ *
+ * with the paper's forward sign -1 and the paper's unitary
+ * scaling c = 1/sqrt(N) by default.  Array index j is the basis
+ * state whose qubit q is bit q of j (q_0 = least-significant bit, PAPER.md:82,
+ * :96); input and output are both in natural order.  For k < n-1 the result is
+ * that of the truncated circuit (the AQFT), which is not the DFT.
+ *
+ * A plan ("planner", fused blocks, device-agnostic schedule)
+ * turns the gate list into a few fused passes over the state.  Each pass loads
+ * a tile of amplitudes, applies every gate whose target lies in the tile's
+ * window of qubits -- Hadamards as butterflies, all controlled-R_m as
+ * per-amplitude phases computed from index bits ("commuting
+ * diagonal factors collapse to one diagonal") -- and stores the tile through a
+ * layout adapter that folds the bit reversal into the
+ * store addressing.  DESIGN.md describes the schedule.
+ *
+ * All functions return a status code; no exception crosses this boundary and
+ * no output argument is written on failure.  No PyTorch type appears here.
+ */
+#ifndef QFT_B200_H
+#define QFT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qft_plan_s* qft_plan_t;
+
+typedef enum {
+    QFT_OK = 0,
+    QFT_ERR_INVALID_ARG = 1, /* null pointer, n out of range, misaligned state, bad sign ... */
+    QFT_ERR_UNSUPPORTED = 2, /* a tuning request the planner cannot schedule */
+    QFT_ERR_ALLOC = 3,       /* host or device allocation failed */
+    QFT_ERR_CUDA = 4,        /* a CUDA runtime call or kernel launch failed (no usable device included) */
+    QFT_ERR_INTERNAL = 5     /* planner self-check failed: a bug, never expected */
+} qft_status_t;
+
+typedef enum {
+    QFT_NORM_UNITARY = 0, /* c = 1/sqrt(N): the paper's U = DFT_N / sqrt(N) */
+    QFT_NORM_NONE = 1,    /* c = 1: plain DFT_N, "multiply by scale_in sqrt(N)" of PAPER.md:139 */
+    QFT_NORM_INV_N = 2    /* c = 1/N: "other FFT conventions ... one-line rescaling" */
+} qft_norm_t;
+
+#define QFT_MAX_QUBITS 34
+
+/*
+ * qft_plan_create -- build the fused schedule (host only; no device is touched,
+ * so it also works on a machine without a GPU).
+ *   out               receives the plan handle.
+ *   n_qubits          1 .. QFT_MAX_QUBITS; the state has 2^n complex64 amplitudes.
+ *   aqft_cutoff_k     >= 0.  Controlled rotations with control-target distance
+ *                     > k are dropped; k >= n-1 is the exact QFT,
+ *                     k = 0 leaves the Hadamards only.
+ *   max_fused_qubits  >= 1.  Cap on the number of logical qubits whose gates one
+ *                     pass applies (the planner's analogue of qsim's
+ *                     max_fused_size).  Values above the device
+ *                     limit (the tile holds 13 qubits, up to 10 of them processed
+ *                     when n > 13) are clamped, not an error.  The result does
+ *                     not depend on it, only the number of passes does.
+ *   sign              -1: the paper's forward transform; +1: every phase
+ *                     conjugated (the inverse DFT when k >= n-1; for k < n-1 it
+ *                     is the conjugated AQFT, not the inverse of the forward AQFT).
+ *   normalisation     see qft_norm_t.
+ */
+qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
+                             qft_norm_t normalisation);
+
+/*
+ * qft_plan_create_tuned -- as qft_plan_create, with the layout knobs exposed for
+ * benchmarking: tile_bits (log2 amplitudes per tile, 0 = default), hub_bits
+ * (log2 amplitudes per contiguous granule, 0 = default), flags (QFT_FLAG_*).
+ * QFT_ERR_UNSUPPORTED if the combination cannot be scheduled.
+ */
+#define QFT_FLAG_GENERIC_ONLY 1u  /* use only the generic shared-memory tile kernel */
+#define QFT_FLAG_UNFOLDED 2u      /* natural-order passes + one stand-alone bit-reversal pass */
+qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
+                                   qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
+
+/*
+ * qft_execute -- enqueue the transform of `device_state` on `stream`, in place.
+ *   device_state  DEVICE pointer to 2^n interleaved (re, im) float pairs, 16-byte
+ *                 aligned (8-byte when n = 0 is not allowed, so always 16), owned
+ *                 by the caller, on the device that is current at the time of the
+ *                 call.  No other 2^n-sized buffer is allocated.
+ *   stream        a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * Only enqueues kernels: no host synchronisation.  The plan is immutable and may
+ * be used again, also on other streams (not concurrently from several threads on
+ * first use, when the small device tables are created).
+ * Errors: QFT_ERR_INVALID_ARG (null / misaligned), QFT_ERR_CUDA (launch failed).
+ */
+qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
+
+/*
+ * qft_execute_host -- the same transform for a state in HOST memory (pageable or
+ * pinned): copies 2^n complex64 to a device buffer owned by the plan (allocated
+ * on first use, 8 * 2^n bytes), runs qft_execute, copies the result back into
+ * `host_state` and waits for it.  This is the end-to-end entry point timed as
+ * "e2e" by bench.py.
+ */
+qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream);
+
+/* qft_plan_destroy -- free the plan and everything it owns.  NULL is allowed. */
+qft_status_t qft_plan_destroy(qft_plan_t plan);
+
+/* Introspection (the paper's plan carries the fused blocks and the counters of
+ * 1- and 2-qubit gates before fusion). */
+int qft_plan_num_passes(qft_plan_t plan);   /* -1 if plan is NULL */
+int qft_plan_num_launches(qft_plan_t plan); /* kernels one qft_execute enqueues; -1 if NULL */
+qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_cr, long long* n_swap);
+/* JSON text describing every pass (window, tile address bits, steps, permutation,
+ * pairing, kernel).  Writes at most len-1 characters plus a NUL; returns
+ * QFT_ERR_INVALID_ARG if the buffer is too small (8 KiB is always enough). */
+qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len);
+/* Re-runs the planner's host-side proof: follows every qubit through every
+ * pass's address permutation and checks that each gate's target was inside the
+ * tile when applied, that tiles are closed under the store permutation, and
+ * that every qubit ends on its bit-reversed address.  QFT_OK or QFT_ERR_INTERNAL. */
+qft_status_t qft_plan_self_check(qft_plan_t plan);
+
+const char* qft_status_string(qft_status_t status);
+/* Last CUDA error text seen by this library on the calling thread ("" if none). */
+const char* qft_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QFT_B200_H */

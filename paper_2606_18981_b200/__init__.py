@@ -1,0 +1,223 @@
+"""Thin Python binding of libqft.so (include/qft.h): argument marshalling only.
+
+Every step of the path (planning, kernels, copies) runs inside the C-ABI
+library; PyTorch appears only in callers, for device memory and streams.  There
+is no CPU fallback: if libqft.so cannot be loaded (and cannot be built because
+nvcc is missing) importing a symbol raises RuntimeError.
+
+Names mirror the C ABI: qft_plan_create, qft_execute, qft_execute_host,
+qft_plan_destroy, qft_plan_num_passes, qft_plan_num_launches,
+qft_plan_gate_counts, qft_plan_describe, qft_plan_self_check,
+qft_status_string.  `Plan` is a small RAII convenience around them.
+"""
+from __future__ import annotations
+
+import ctypes
+import json
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqft.so")
+
+QFT_OK, QFT_ERR_INVALID_ARG, QFT_ERR_UNSUPPORTED, QFT_ERR_ALLOC, QFT_ERR_CUDA, QFT_ERR_INTERNAL = range(6)
+QFT_NORM_UNITARY, QFT_NORM_NONE, QFT_NORM_INV_N = 0, 1, 2
+QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED = 1, 2
+QFT_MAX_QUBITS = 34
+
+EXPORTS = [
+    "qft_plan_create", "qft_plan_create_tuned", "qft_execute", "qft_execute_host", "qft_plan_destroy",
+    "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
+    "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
+]
+
+_lib = None
+
+
+class QftError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = qft_status_string(status)
+        detail = qft_last_cuda_error()
+        super().__init__(f"{where}: {msg}" + (f" ({detail})" if detail else ""))
+
+
+def load() -> ctypes.CDLL:
+    """Load libqft.so; build it first if it is missing and nvcc is available."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        try:
+            from . import build as _build
+
+            _build.build()
+        except Exception as exc:  # no nvcc, compile error ...
+            raise RuntimeError(
+                f"libqft.so is missing at {LIB_PATH} and could not be built ({exc}); "
+                "there is no CPU fallback for the QFT path") from exc
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    L.qft_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci]
+    L.qft_plan_create.restype = ci
+    L.qft_plan_create_tuned.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ci, ci, ctypes.c_uint]
+    L.qft_plan_create_tuned.restype = ci
+    L.qft_execute.argtypes = [vp, vp, vp]
+    L.qft_execute.restype = ci
+    L.qft_execute_host.argtypes = [vp, vp, vp]
+    L.qft_execute_host.restype = ci
+    L.qft_plan_destroy.argtypes = [vp]
+    L.qft_plan_destroy.restype = ci
+    L.qft_plan_num_passes.argtypes = [vp]
+    L.qft_plan_num_passes.restype = ci
+    L.qft_plan_num_launches.argtypes = [vp]
+    L.qft_plan_num_launches.restype = ci
+    llp = ctypes.POINTER(ctypes.c_longlong)
+    L.qft_plan_gate_counts.argtypes = [vp, llp, llp, llp]
+    L.qft_plan_gate_counts.restype = ci
+    L.qft_plan_describe.argtypes = [vp, ctypes.c_char_p, ctypes.c_size_t]
+    L.qft_plan_describe.restype = ci
+    L.qft_plan_self_check.argtypes = [vp]
+    L.qft_plan_self_check.restype = ci
+    L.qft_status_string.argtypes = [ci]
+    L.qft_status_string.restype = ctypes.c_char_p
+    L.qft_last_cuda_error.argtypes = []
+    L.qft_last_cuda_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+# ---- one-to-one wrappers (raise QftError on a non-zero status) ---------------------------------
+
+def qft_status_string(status: int) -> str:
+    return load().qft_status_string(int(status)).decode()
+
+
+def qft_last_cuda_error() -> str:
+    return load().qft_last_cuda_error().decode()
+
+
+def qft_plan_create(n_qubits: int, aqft_cutoff_k: int, max_fused_qubits: int = 13, sign: int = -1,
+                    normalisation: int = QFT_NORM_UNITARY) -> int:
+    h = ctypes.c_void_p()
+    st = load().qft_plan_create(ctypes.byref(h), n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation)
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_create")
+    return h.value
+
+
+def qft_plan_create_tuned(n_qubits: int, aqft_cutoff_k: int, max_fused_qubits: int = 13, sign: int = -1,
+                          normalisation: int = QFT_NORM_UNITARY, tile_bits: int = 0, hub_bits: int = 0,
+                          flags: int = 0) -> int:
+    h = ctypes.c_void_p()
+    st = load().qft_plan_create_tuned(ctypes.byref(h), n_qubits, aqft_cutoff_k, max_fused_qubits, sign,
+                                      normalisation, tile_bits, hub_bits, flags)
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_create_tuned")
+    return h.value
+
+
+def qft_execute(plan: int, device_state_ptr: int, stream: int = 0) -> None:
+    st = load().qft_execute(plan, device_state_ptr, stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_execute")
+
+
+def qft_execute_host(plan: int, host_state_ptr: int, stream: int = 0) -> None:
+    st = load().qft_execute_host(plan, host_state_ptr, stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_execute_host")
+
+
+def qft_plan_destroy(plan: int) -> None:
+    load().qft_plan_destroy(plan)
+
+
+def qft_plan_num_passes(plan: int) -> int:
+    return int(load().qft_plan_num_passes(plan))
+
+
+def qft_plan_num_launches(plan: int) -> int:
+    return int(load().qft_plan_num_launches(plan))
+
+
+def qft_plan_gate_counts(plan: int):
+    a, b, c = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_longlong()
+    st = load().qft_plan_gate_counts(plan, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c))
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_gate_counts")
+    return a.value, b.value, c.value
+
+
+def qft_plan_describe(plan: int) -> dict:
+    buf = ctypes.create_string_buffer(1 << 16)
+    st = load().qft_plan_describe(plan, buf, len(buf))
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_describe")
+    return json.loads(buf.value.decode())
+
+
+def qft_plan_self_check(plan: int) -> None:
+    st = load().qft_plan_self_check(plan)
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_self_check")
+
+
+class Plan:
+    """RAII wrapper: Plan(n, k).execute(tensor) transforms a CUDA complex64 tensor in place."""
+
+    def __init__(self, n_qubits: int, aqft_cutoff_k: int | None = None, max_fused_qubits: int = 13, sign: int = -1,
+                 normalisation: int = QFT_NORM_UNITARY, tile_bits: int = 0, hub_bits: int = 0, flags: int = 0):
+        if aqft_cutoff_k is None:
+            aqft_cutoff_k = n_qubits
+        self.n = n_qubits
+        self.handle = qft_plan_create_tuned(n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation,
+                                            tile_bits, hub_bits, flags)
+
+    def execute(self, state, stream: int | None = None) -> None:
+        """state: torch complex64 CUDA tensor of 2^n elements (contiguous).  In place, asynchronous."""
+        import torch
+
+        if state.dtype != torch.complex64 or not state.is_cuda or not state.is_contiguous() or \
+                state.numel() != (1 << self.n):
+            raise ValueError("state must be a contiguous CUDA complex64 tensor of 2^n elements")
+        if stream is None:
+            stream = torch.cuda.current_stream(state.device).cuda_stream
+        qft_execute(self.handle, state.data_ptr(), stream)
+
+    def execute_host(self, state, stream: int = 0) -> None:
+        """state: numpy complex64 array or CPU torch tensor of 2^n elements; in place, synchronous."""
+        if hasattr(state, "data_ptr"):
+            ptr, cnt = state.data_ptr(), state.numel()
+        else:
+            ptr, cnt = state.ctypes.data, state.size
+        if cnt != (1 << self.n):
+            raise ValueError("state must hold 2^n complex64 elements")
+        qft_execute_host(self.handle, ptr, stream)
+
+    @property
+    def num_passes(self) -> int:
+        return qft_plan_num_passes(self.handle)
+
+    @property
+    def num_launches(self) -> int:
+        return qft_plan_num_launches(self.handle)
+
+    def gate_counts(self):
+        return qft_plan_gate_counts(self.handle)
+
+    def describe(self) -> dict:
+        return qft_plan_describe(self.handle)
+
+    def self_check(self) -> None:
+        qft_plan_self_check(self.handle)
+
+    def close(self) -> None:
+        if getattr(self, "handle", None):
+            qft_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,158 @@
+// qft_api.cu -- the C ABI declared in include/qft.h.
+#include <cuda_runtime.h>
+
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/qft.h"
+#include "qft_plan.h"
+
+cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream);
+
+struct qft_plan_s {
+    QftHostPlan host;
+    void* dev_buf = nullptr;  // only for qft_execute_host
+    size_t dev_bytes = 0;
+};
+
+static thread_local std::string g_cuda_err;
+
+static qft_status_t cuda_fail(cudaError_t e) {
+    g_cuda_err = cudaGetErrorString(e);
+    return QFT_ERR_CUDA;
+}
+
+extern "C" {
+
+qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
+                                   qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags) {
+    if (!out) return QFT_ERR_INVALID_ARG;
+    QftPlanParams prm;
+    prm.n = n_qubits;
+    prm.k = aqft_cutoff_k;
+    prm.max_fused = max_fused_qubits;
+    prm.sign = sign;
+    prm.norm = (int)normalisation;
+    prm.tile_bits = tile_bits;
+    prm.hub_bits = hub_bits;
+    prm.flags = flags;
+    qft_plan_s* p = new (std::nothrow) qft_plan_s();
+    if (!p) return QFT_ERR_ALLOC;
+    std::string err;
+    int rc;
+    try {
+        rc = qft_build_plan(prm, &p->host, &err);
+    } catch (const std::bad_alloc&) {
+        delete p;
+        return QFT_ERR_ALLOC;
+    } catch (...) {
+        delete p;
+        return QFT_ERR_INTERNAL;
+    }
+    if (rc != 0) {
+        delete p;
+        g_cuda_err = err;
+        return (qft_status_t)rc;
+    }
+    *out = p;
+    return QFT_OK;
+}
+
+qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
+                             qft_norm_t normalisation) {
+    return qft_plan_create_tuned(out, n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation, 0, 0, 0u);
+}
+
+qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream) {
+    if (!plan || !device_state) return QFT_ERR_INVALID_ARG;
+    const uintptr_t align = plan->host.prm.n >= 1 ? 16 : 8;
+    if (((uintptr_t)device_state) & (align - 1)) return QFT_ERR_INVALID_ARG;
+    for (const QftPassDesc& d : plan->host.passes) {
+        cudaError_t e = qft_launch_pass(d, device_state, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return QFT_OK;
+}
+
+qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream) {
+    if (!plan || !host_state) return QFT_ERR_INVALID_ARG;
+    const size_t bytes = (size_t)8 << plan->host.prm.n;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!plan->dev_buf) {
+        cudaError_t e = cudaMalloc(&plan->dev_buf, bytes);
+        if (e != cudaSuccess) {
+            plan->dev_buf = nullptr;
+            g_cuda_err = cudaGetErrorString(e);
+            return e == cudaErrorMemoryAllocation ? QFT_ERR_ALLOC : QFT_ERR_CUDA;
+        }
+        plan->dev_bytes = bytes;
+    }
+    cudaError_t e = cudaMemcpyAsync(plan->dev_buf, host_state, bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    qft_status_t st = qft_execute(plan, plan->dev_buf, stream);
+    if (st != QFT_OK) return st;
+    e = cudaMemcpyAsync(host_state, plan->dev_buf, bytes, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return QFT_OK;
+}
+
+qft_status_t qft_plan_destroy(qft_plan_t plan) {
+    if (!plan) return QFT_OK;
+    if (plan->dev_buf) cudaFree(plan->dev_buf);
+    delete plan;
+    return QFT_OK;
+}
+
+int qft_plan_num_passes(qft_plan_t plan) { return plan ? (int)plan->host.passes.size() : -1; }
+int qft_plan_num_launches(qft_plan_t plan) { return plan ? (int)plan->host.passes.size() : -1; }
+
+qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_cr, long long* n_swap) {
+    if (!plan || !n_h || !n_cr || !n_swap) return QFT_ERR_INVALID_ARG;
+    *n_h = plan->host.n_h;
+    *n_cr = plan->host.n_cr;
+    *n_swap = plan->host.n_swap;
+    return QFT_OK;
+}
+
+qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len) {
+    if (!plan || !buf || len == 0) return QFT_ERR_INVALID_ARG;
+    std::string s;
+    try {
+        s = qft_describe_plan(plan->host);
+    } catch (...) {
+        return QFT_ERR_ALLOC;
+    }
+    if (s.size() + 1 > len) return QFT_ERR_INVALID_ARG;
+    std::memcpy(buf, s.c_str(), s.size() + 1);
+    return QFT_OK;
+}
+
+qft_status_t qft_plan_self_check(qft_plan_t plan) {
+    if (!plan) return QFT_ERR_INVALID_ARG;
+    std::string err;
+    int rc = qft_check_plan(plan->host, &err);
+    if (rc != 0) {
+        g_cuda_err = err;
+        return QFT_ERR_INTERNAL;
+    }
+    return QFT_OK;
+}
+
+const char* qft_status_string(qft_status_t status) {
+    switch (status) {
+        case QFT_OK: return "ok";
+        case QFT_ERR_INVALID_ARG: return "invalid argument";
+        case QFT_ERR_UNSUPPORTED: return "unsupported";
+        case QFT_ERR_ALLOC: return "allocation failed";
+        case QFT_ERR_CUDA: return "CUDA error";
+        case QFT_ERR_INTERNAL: return "internal planner error";
+    }
+    return "unknown status";
+}
+
+const char* qft_last_cuda_error(void) { return g_cuda_err.c_str(); }
+
+}  // extern "C"

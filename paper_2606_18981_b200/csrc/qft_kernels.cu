@@ -1,0 +1,185 @@
+// qft_kernels.cu -- the pass kernels (sm_100a) and their launcher.
+//
+// Generic tile pass (QFT_KERNEL_GENERIC): works for every pass descriptor the planner can emit.
+//   1. load the tile (all addresses that agree outside F) into shared memory in canonical order,
+//      one 8-byte amplitude per lane, lanes running along the hub so that every warp request covers
+//      whole 2^l * 8-byte granules;
+//   2. for each step, every thread takes 2^r amplitudes that differ in the step's r canonical bits,
+//      applies H and all controlled rotations onto those r qubits (register butterflies with constant
+//      twiddles for controls inside the group, index-bit phases for controls outside it:
+//      PAPER.md:112, :114), and puts them back;
+//   3. store through the pass's layout adapter: canonical bit -> address bit
+//      permutation inside the tile and, for pair passes, into the partner tile's addresses after a
+//      cluster barrier (both CTAs of the pair have finished loading by then, so in place is safe).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "qft_device.cuh"
+#include "qft_plan.h"
+
+namespace qftk {
+
+// bank swizzle of the shared-memory image (any bijection is correct; this one spreads strided steps)
+__device__ __forceinline__ uint32_t swz(uint32_t c) { return c ^ ((c >> 4) & 0xFu) ^ ((c >> 8) & 0xFu); }
+
+template <int R, bool FAST>
+__device__ __forceinline__ void generic_step(float2* tile, const QftPassDesc& d, const QftStep st, uint64_t Ltile,
+                                             bool scale_now) {
+    const int a = st.a;
+    const int t_hi = st.t_hi;
+    const int t_lo = t_hi - R + 1;
+    const uint32_t nb = 1u << (d.f - R);
+    const uint32_t lowmask = (1u << a) - 1u;
+    const uint64_t lmask = (t_lo > 0) ? ((1ull << t_lo) - 1ull) : 0ull;
+    for (uint32_t o = threadIdx.x; o < nb; o += blockDim.x) {
+        const uint32_t c0 = ((o & ~lowmask) << R) | (o & lowmask);
+        float2 x[1 << R];
+#pragma unroll
+        for (int u = 0; u < (1 << R); ++u) x[u] = tile[swz(c0 | ((uint32_t)u << a))];
+        dif_group<R, FAST>(x, d.k);
+        if (t_lo > 0) {
+            // logical bits below the group: from the tile index and from this thread's canonical low bits
+            uint64_t L = Ltile;
+            for (int b = 0; b < a; ++b)
+                if ((c0 >> b) & 1u) L |= 1ull << d.log_canon[b];
+            L &= lmask;
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                const float2 W = cis_fwd_u32(cr_phase_u32(L, t_hi - i, d.k));
+                constexpr int dummy = 0;
+                (void)dummy;
+                const int pos = R - 1 - i;
+#pragma unroll
+                for (int u = 0; u < (1 << R); ++u)
+                    if (u & (1 << pos)) x[u] = cmul(x[u], W);
+            }
+        }
+        if (scale_now) {
+#pragma unroll
+            for (int u = 0; u < (1 << R); ++u) { x[u].x *= d.scale; x[u].y *= d.scale; }
+        }
+#pragma unroll
+        for (int u = 0; u < (1 << R); ++u) tile[swz(c0 | ((uint32_t)u << a))] = x[u];
+    }
+}
+
+template <int R>
+__device__ __forceinline__ void generic_step_dispatch(float2* tile, const QftPassDesc& d, const QftStep st,
+                                                      uint64_t Ltile, bool scale_now) {
+    if (d.k >= R - 1) generic_step<R, true>(tile, d, st, Ltile, scale_now);
+    else generic_step<R, false>(tile, d, st, Ltile, scale_now);
+}
+
+__global__ void __launch_bounds__(256) qft_tile_pass_generic(float2* __restrict__ state,
+                                                             const __grid_constant__ QftPassDesc d) {
+    extern __shared__ float2 tile[];
+    const uint32_t tid = threadIdx.x;
+    const int lt = d.log2_threads;
+
+    uint32_t mload, mstore;
+    decode_tile(blockIdx.x, d.npair, &mload, &mstore);
+    uint64_t base_ld = 0, base_st = 0, Ltile = 0;
+    for (int i = 0; i < d.ntile; ++i) {
+        if ((mload >> i) & 1u) {
+            base_ld |= 1ull << d.tile_addr[i];
+            Ltile |= 1ull << d.log_tile[i];
+        }
+        if ((mstore >> i) & 1u) base_st |= 1ull << d.tile_addr[i];
+    }
+
+    // ---- load ----
+    {
+        uint64_t off_t = 0;
+        uint32_t can_t = 0;
+        for (int j = 0; j < lt && j < d.f; ++j)
+            if ((tid >> j) & 1u) { off_t |= 1ull << d.F[j]; can_t |= 1u << d.ld_canon[j]; }
+        const uint32_t niter = (d.f > lt) ? (1u << (d.f - lt)) : 1u;
+        const bool active = (d.f >= lt) || (tid < (1u << d.f));
+        if (active) {
+            for (uint32_t it = 0; it < niter; ++it) {
+                uint64_t off = off_t;
+                uint32_t can = can_t;
+                for (int j = lt; j < d.f; ++j)
+                    if ((it >> (j - lt)) & 1u) { off |= 1ull << d.F[j]; can |= 1u << d.ld_canon[j]; }
+                float2 v = state[base_ld + off];
+                if (d.conj) v.y = -v.y;
+                tile[swz(can)] = v;
+            }
+        }
+    }
+    __syncthreads();
+    if (d.npair) cluster_arrive();  // this CTA has read its whole tile
+
+    // ---- steps ----
+    for (int s = 0; s < d.nsteps; ++s) {
+        const QftStep st = d.steps[s];
+        const bool scale_now = d.do_scale && (s == d.nsteps - 1);
+        switch (st.r) {
+            case 1: generic_step_dispatch<1>(tile, d, st, Ltile, scale_now); break;
+            case 2: generic_step_dispatch<2>(tile, d, st, Ltile, scale_now); break;
+            case 3: generic_step_dispatch<3>(tile, d, st, Ltile, scale_now); break;
+            case 4: generic_step_dispatch<4>(tile, d, st, Ltile, scale_now); break;
+            default: generic_step_dispatch<5>(tile, d, st, Ltile, scale_now); break;
+        }
+        __syncthreads();
+    }
+    if (d.npair) cluster_wait();  // the partner has read its tile: its addresses may be overwritten
+
+    // ---- store ----
+    {
+        uint64_t off_t = 0;
+        uint32_t can_t = 0;
+        for (int j = 0; j < lt && j < d.f; ++j)
+            if ((tid >> j) & 1u) { off_t |= 1ull << d.F[j]; can_t |= 1u << d.st_canon[j]; }
+        const uint32_t niter = (d.f > lt) ? (1u << (d.f - lt)) : 1u;
+        const bool active = (d.f >= lt) || (tid < (1u << d.f));
+        if (active) {
+            for (uint32_t it = 0; it < niter; ++it) {
+                uint64_t off = off_t;
+                uint32_t can = can_t;
+                for (int j = lt; j < d.f; ++j)
+                    if ((it >> (j - lt)) & 1u) { off |= 1ull << d.F[j]; can |= 1u << d.st_canon[j]; }
+                float2 v = tile[swz(can)];
+                if (d.conj) v.y = -v.y;
+                state[base_st + off] = v;
+            }
+        }
+    }
+}
+
+}  // namespace qftk
+
+// ---------------------------------------------------------------------------------------------
+// launcher
+// ---------------------------------------------------------------------------------------------
+static cudaError_t ensure_attrs() {
+    static bool done = false;
+    static cudaError_t st = cudaSuccess;
+    if (!done) {
+        st = cudaFuncSetAttribute(qftk::qft_tile_pass_generic, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  8 << QFT_MAX_TILE_BITS);
+        if (st == cudaSuccess) done = true;
+    }
+    return st;
+}
+
+cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream) {
+    cudaError_t e = ensure_attrs();
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1u << d.ntile);
+    cfg.blockDim = dim3(1u << d.log2_threads);
+    cfg.dynamicSmemBytes = (size_t)8 << d.f;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    cfg.attrs = attr;
+    cfg.numAttrs = 0;
+    if (d.npair > 0) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.numAttrs = 1;
+    }
+    return cudaLaunchKernelEx(&cfg, qftk::qft_tile_pass_generic, (float2*)state, d);
+}

@@ -1,0 +1,87 @@
+// qft_plan.h -- pass descriptors shared by the host planner and the kernels.
+//
+// Vocabulary (DESIGN.md has the full story):
+//   address bit a   : bit a of the array index of an amplitude in HBM.
+//   logical qubit q : the circuit's wire q_q; pos[q] is the address
+//                     bit that currently holds it.  Initially pos[q] = q; after
+//                     the last pass pos[q] = n-1-q (the bit reversal).
+//   tile            : all addresses that agree outside a set F of f address bits.
+//                     F always contains the hub [0, l) so that every global access
+//                     moves whole 2^l * 8-byte granules.
+//   canonical bit c : position inside the tile's shared-memory image; canonical
+//                     bits are ordered by the logical qubit they hold, so a window
+//                     of consecutive logical qubits is a run of canonical bits.
+//   window          : the logical qubits whose gates (H and every controlled-R_m
+//                     that targets them) this pass applies.
+//   step            : a group of <= 5 window qubits transformed in registers
+//                     (radix-2^r butterfly) between shared-memory exchanges.
+#pragma once
+#include <stdint.h>
+
+#define QFT_MAX_TILE_BITS 14
+#define QFT_MAX_TILEIDX_BITS 34
+#define QFT_MAX_STEPS 14
+#define QFT_MAX_RADIX_BITS 5
+
+struct QftStep {
+    int8_t r;     // qubits in the group
+    int8_t a;     // lowest canonical bit of the group: canonical bits [a, a+r)
+    int8_t t_hi;  // logical qubit on canonical bit a+r-1 (the first one processed)
+    int8_t pad;
+};
+
+enum QftKernelKind : int32_t {
+    QFT_KERNEL_GENERIC = 0,  // shared-memory staged tile pass, any descriptor
+    QFT_KERNEL_FUSED2 = 1,   // two register steps: global -> reg -> smem -> reg -> global
+};
+
+// Plain data, passed to the kernels by value (__grid_constant__).
+struct QftPassDesc {
+    int32_t n;          // qubits
+    int32_t f;          // tile bits
+    int32_t ntile;      // n - f
+    int32_t npair;      // p: tile-index bits [0,p) trade places with bits [p,2p) on store
+    int32_t nsteps;
+    int32_t k;          // AQFT cutoff (clamped to n)
+    int32_t conj;       // sign = +1: conjugate on load and on store
+    int32_t kernel;     // QftKernelKind
+    int32_t log2_threads;
+    float scale;        // applied in the last step (1 unless this is the final pass)
+    int32_t do_scale;
+    int32_t win_lo;     // lowest logical qubit of the window (-1: permutation-only pass)
+    int8_t F[16];         // load/store-order bit j <-> address bit F[j], ascending, F[j] = j for j < l
+    int8_t ld_canon[16];  // load-order bit j  -> canonical bit
+    int8_t st_canon[16];  // store-order bit j -> canonical bit whose data lands on address F[j]
+    int8_t log_canon[16]; // canonical bit -> logical qubit
+    int8_t tile_addr[QFT_MAX_TILEIDX_BITS];  // tile-index bit -> address bit
+    int8_t log_tile[QFT_MAX_TILEIDX_BITS];   // tile-index bit -> logical qubit held at load time
+    QftStep steps[QFT_MAX_STEPS];
+};
+
+#include <string>
+#include <vector>
+
+struct QftPlanParams {
+    int n = 0;
+    int k = 0;
+    int max_fused = 0;
+    int sign = -1;
+    int norm = 0;
+    int tile_bits = 0;  // 0 = default
+    int hub_bits = 0;   // 0 = default
+    unsigned flags = 0;
+};
+
+struct QftHostPlan {
+    QftPlanParams prm;
+    int k_eff = 0;  // min(k, n)
+    int tile_bits = 0, hub_bits = 0, window = 0;
+    bool folded = false;
+    std::vector<QftPassDesc> passes;
+    long long n_h = 0, n_cr = 0, n_swap = 0;
+};
+
+// Returns 0 (ok), 1 (invalid argument), 2 (unsupported tuning), 5 (internal: self-check failed).
+int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err);
+int qft_check_plan(const QftHostPlan& plan, std::string* err);
+std::string qft_describe_plan(const QftHostPlan& plan);

@@ -1,0 +1,178 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances are north_star's: relative L2 error <= 2e-5 for n <= 20 and <= 1e-4 up to n = 33.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import qft_inputs as qi
+
+pytestmark = pytest.mark.gpu
+
+TOL_SMALL = 2e-5   # n <= 20 (north_star)
+TOL_LARGE = 1e-4   # n <= 33 (north_star)
+
+
+def tol(n):
+    return TOL_SMALL if n <= 20 else TOL_LARGE
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.complex128)
+    b = np.asarray(b, dtype=np.complex128)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def gpu_qft(x, k=None, **kw):
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    n = int(x.shape[0]).bit_length() - 1
+    plan = qft.Plan(n, n if k is None else k, **kw)
+    plan.self_check()
+    t = torch.from_numpy(np.ascontiguousarray(x, dtype=np.complex64)).cuda()
+    plan.execute(t)
+    torch.cuda.synchronize()
+    out = t.cpu().numpy()
+    plan.close()
+    return out
+
+
+@pytest.mark.parametrize("n", list(range(1, 17)))
+def test_exact_small_n(n):
+    x = qi.gaussian(n, 40 + n)
+    assert rel_l2(gpu_qft(x), oracle.qft(x)) <= tol(n)
+
+
+def test_config1_n10():
+    """BASELINE config 1: n = 10, Gaussian seed 0, forward, unitary."""
+    x = qi.gaussian(10, 0)
+    got = gpu_qft(x)
+    assert rel_l2(got, oracle.qft(x)) <= TOL_SMALL
+    assert rel_l2(got, oracle.naive_dft(x)) <= TOL_SMALL
+
+
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4, 5, 8, 11, 12])
+@pytest.mark.parametrize("n", [7, 12, 15])
+def test_aqft_cutoffs(n, k):
+    x = qi.gaussian(n, 7 * n + k)
+    assert rel_l2(gpu_qft(x, k), oracle.qft(x, k)) <= tol(n)
+
+
+@pytest.mark.parametrize("sign", [-1, 1])
+@pytest.mark.parametrize("norm", [0, 1, 2])
+def test_sign_and_normalisation(sign, norm):
+    for n, k in ((9, 9), (14, 14), (14, 3)):
+        x = qi.gaussian(n, 3)
+        assert rel_l2(gpu_qft(x, k, sign=sign, normalisation=norm), oracle.qft(x, k, sign, norm)) <= tol(n)
+
+
+@pytest.mark.parametrize("w", [1, 2, 3, 4, 6, 9, 10, 13])
+@pytest.mark.parametrize("n", [11, 16, 18])
+def test_result_independent_of_max_fused_qubits(n, w):
+    x = qi.gaussian(n, 5)
+    ref = oracle.qft(x, 6)
+    assert rel_l2(gpu_qft(x, 6, max_fused_qubits=w), ref) <= tol(n)
+
+
+@pytest.mark.parametrize("tile_bits,hub_bits", [(4, 1), (5, 2), (6, 2), (7, 3), (9, 3), (12, 4), (14, 3), (14, 4)])
+def test_tuned_layouts(tile_bits, hub_bits):
+    """Small tiles force many passes, pair (cluster) passes and ragged windows at small n."""
+    for n in (5, 8, 11, 13, 15, 17):
+        for flags in (0, 2):
+            for k in (n, 3):
+                x = qi.gaussian(n, n)
+                got = gpu_qft(x, k, tile_bits=tile_bits, hub_bits=hub_bits, flags=flags)
+                assert rel_l2(got, oracle.qft(x, k)) <= tol(n), (n, flags, k)
+
+
+def test_config2_n20_three_inputs():
+    n, N = 20, 1 << 20
+    xg = qi.gaussian(n, 0)
+    assert rel_l2(gpu_qft(xg), oracle.qft(xg)) <= TOL_SMALL
+    xt = qi.tone(n, 12345)
+    got = gpu_qft(xt)
+    assert rel_l2(got, oracle.qft(xt)) <= TOL_SMALL
+    assert abs(abs(got[12345]) - 1.0) < 1e-4 and np.linalg.norm(np.delete(got, 12345)) < 1e-3
+    xd = qi.delta(n, 777)
+    got = gpu_qft(xd)
+    assert rel_l2(got, oracle.qft(xd)) <= TOL_SMALL
+    K = np.arange(N)
+    want = np.exp(-2j * np.pi * ((777 * K) % N) / N) / 1024.0
+    assert rel_l2(got, want) <= TOL_SMALL
+
+
+def test_paper_workload_n22_tone2():
+    """The paper's own correctness input: single tone at bin k0 = 2, n = 22."""
+    n = 22
+    x = qi.tone(n, 2)
+    got = gpu_qft(x)
+    assert rel_l2(got, oracle.qft(x)) <= TOL_LARGE
+    for k in (4, 8):
+        gk = gpu_qft(x, k)
+        assert rel_l2(gk, oracle.qft(x, k)) <= TOL_LARGE
+        leak = 1 - abs(gk[2]) ** 2 / float(np.vdot(gk, gk).real)
+        pred = (4 * np.pi ** 2 / 3) * 4.0 ** (-(k + 2))
+        assert 0.5 * pred < leak < 2.0 * pred
+
+
+def test_linearity_and_round_trip_on_device():
+    n = 17
+    a, b = qi.gaussian(n, 1), qi.gaussian(n, 2)
+    al, be = np.complex64(0.3 - 1.1j), np.complex64(-2.0 + 0.25j)
+    lhs = gpu_qft((al * a + be * b).astype(np.complex64), 5)
+    rhs = al * gpu_qft(a, 5) + be * gpu_qft(b, 5)
+    assert rel_l2(lhs, rhs) <= 1e-5
+    back = gpu_qft(gpu_qft(a), sign=1)
+    assert rel_l2(back, a) <= 1e-5
+
+
+def test_execute_host_matches_device_path():
+    import paper_2606_18981_b200 as qft
+
+    n = 16
+    x = qi.gaussian(n, 8)
+    h = x.copy()
+    plan = qft.Plan(n, 7)
+    plan.execute_host(h)
+    plan.close()
+    assert rel_l2(h, oracle.qft(x, 7)) <= TOL_SMALL
+
+
+def test_plan_reuse_and_streams():
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    n = 15
+    plan = qft.Plan(n, n)
+    s = torch.cuda.Stream()
+    xs = [qi.gaussian(n, i) for i in range(3)]
+    outs = []
+    for x in xs:
+        t = torch.from_numpy(x).cuda()
+        with torch.cuda.stream(s):
+            plan.execute(t)
+        s.synchronize()
+        outs.append(t.cpu().numpy())
+    for x, o in zip(xs, outs):
+        assert rel_l2(o, oracle.qft(x)) <= TOL_SMALL
+    plan.close()
+
+
+def test_error_codes_on_device():
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    plan = qft.Plan(8, 8)
+    t = torch.zeros(256 + 1, dtype=torch.complex64, device="cuda")
+    with pytest.raises(qft.QftError):
+        qft.qft_execute(plan.handle, t.data_ptr() + 8, 0)  # misaligned
+    with pytest.raises(qft.QftError):
+        qft.qft_execute(plan.handle, 0, 0)  # null
+    plan.close()

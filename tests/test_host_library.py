@@ -1,0 +1,128 @@
+"""CPU-only checks of libqft.so: it loads, exports every symbol of include/qft.h, validates
+arguments, and its planner's schedules pass the host-side proof (no kernel is launched here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2606_18981_b200 as qft
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "qft.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(qft_[a-z_]+)\s*\(", hdr))
+    assert {"qft_plan_create", "qft_execute", "qft_plan_destroy"} <= declared
+    lib = ctypes.CDLL(qft.LIB_PATH)
+    for name in sorted(declared):
+        assert hasattr(lib, name), name
+    assert declared == set(qft.EXPORTS)
+
+
+def test_status_strings():
+    assert qft.qft_status_string(0) == "ok"
+    for s in range(1, 6):
+        assert qft.qft_status_string(s) not in ("ok", "unknown status")
+
+
+@pytest.mark.parametrize("args", [
+    (0, 1, 13, -1, 0), (35, 1, 13, -1, 0), (10, -1, 13, -1, 0), (10, 3, 0, -1, 0), (10, 3, 13, 0, 0),
+    (10, 3, 13, 2, 0), (10, 3, 13, -1, 3), (10, 3, 13, -1, -1),
+])
+def test_invalid_arguments(args):
+    with pytest.raises(qft.QftError) as e:
+        qft.qft_plan_create(*args)
+    assert e.value.status == qft.QFT_ERR_INVALID_ARG
+
+
+def test_null_out_pointer_and_null_plan():
+    L = qft.load()
+    assert L.qft_plan_create(None, 10, 10, 13, -1, 0) == qft.QFT_ERR_INVALID_ARG
+    assert L.qft_execute(None, None, None) == qft.QFT_ERR_INVALID_ARG
+    assert L.qft_plan_num_passes(None) == -1
+    assert L.qft_plan_destroy(None) == qft.QFT_OK
+    h = qft.qft_plan_create(10, 10)
+    assert L.qft_execute(h, None, None) == qft.QFT_ERR_INVALID_ARG
+    assert L.qft_execute(h, ctypes.c_void_p(8), None) == qft.QFT_ERR_INVALID_ARG  # misaligned
+    small = ctypes.create_string_buffer(8)
+    assert L.qft_plan_describe(h, small, 8) == qft.QFT_ERR_INVALID_ARG
+    qft.qft_plan_destroy(h)
+
+
+def test_unsupported_tuning():
+    with pytest.raises(qft.QftError) as e:
+        qft.qft_plan_create_tuned(10, 10, 13, -1, 0, tile_bits=15)
+    assert e.value.status == qft.QFT_ERR_UNSUPPORTED
+    with pytest.raises(qft.QftError):
+        qft.qft_plan_create_tuned(34, 10, 13, -1, 0, tile_bits=2, hub_bits=1)
+
+
+def test_gate_counters_table2():
+    """The plan carries the 1- and 2-qubit gate counters before fusion;
+    Table 2 fixes the controlled-R_m count at n = 22."""
+    with open(os.path.join(GOLD, "table2_cr_counts_n22.txt")) as fh:
+        rows = [tuple(l.split()) for l in fh if l.strip() and not l.startswith("#")]
+    for k, cnt, _ in rows:
+        p = qft.Plan(22, int(k))
+        assert p.gate_counts() == (22, int(cnt), 11)
+        p.close()
+    p = qft.Plan(30, 30)
+    assert p.gate_counts() == (30, 435, 15)
+    p.close()
+    p = qft.Plan(33, 16)
+    assert p.gate_counts() == (33, 392, 16)
+    p.close()
+
+
+@pytest.mark.parametrize("n", list(range(1, 35)))
+def test_every_schedule_passes_the_host_proof(n):
+    for w in (1, 2, 3, 4, 6, 10, 13, 40):
+        for flags in (0, qft.QFT_FLAG_UNFOLDED):
+            p = qft.Plan(n, n, w, flags=flags)
+            p.self_check()
+            d = p.describe()
+            assert d["n"] == n and len(d["passes"]) == p.num_passes
+            done = []
+            for ps in d["passes"]:
+                assert len(ps["window"]) <= max(1, min(w, 13))
+                done += ps["window"]
+            assert done == list(range(n - 1, -1, -1))  # circuit order, every qubit once
+            p.close()
+
+
+@pytest.mark.parametrize("tile_bits,hub_bits", [(4, 1), (5, 2), (6, 2), (7, 3), (9, 3), (12, 4), (14, 3), (14, 4)])
+def test_tuned_schedules_pass_the_host_proof(tile_bits, hub_bits):
+    for n in range(1, 31):
+        for w in (1, 3, 13):
+            for flags in (0, qft.QFT_FLAG_UNFOLDED):
+                p = qft.Plan(n, 5, w, tile_bits=tile_bits, hub_bits=hub_bits, flags=flags)
+                p.self_check()
+                p.close()
+
+
+def test_pass_counts_at_the_bench_configs():
+    """Folded schedule: ceil(n / window) passes with no stand-alone bit-reversal pass."""
+    want = {10: 1, 13: 1, 20: 3, 26: 3, 30: 3, 33: 4}
+    for n, passes in want.items():
+        p = qft.Plan(n, n)
+        assert p.num_passes == passes, n
+        assert p.num_launches == passes
+        p.close()
+    # config 3: sweep of max_fused_qubits at n = 26
+    got = []
+    for w in (2, 4, 6, 10, 13):
+        p = qft.Plan(26, 26, w)
+        got.append(p.num_passes)
+        p.close()
+    assert got == sorted(got, reverse=True) and got[-1] == 3
+
+
+def test_k_is_clamped_and_reported():
+    p = qft.Plan(12, 1000)
+    assert p.describe()["k"] == 12
+    assert p.gate_counts()[1] == 66
+    p.close()

@@ -1,0 +1,433 @@
+#!/usr/bin/env python
+"""bench.py -- QFT time / DFT-equivalent GFLOP/s / HBM roofline on B200 (BASELINE.json's metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 30] [--k K] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: one qft_execute (every fused pass, the folded bit
+reversal and the normalisation) over one synthetic 2^n complex64 state that is already resident in
+HBM.  Default workload: n = 30 exact QFT (BASELINE config 4 with k = 30: 8 GiB state, the largest
+configuration whose full parity check also runs in the test suite; n = 33 is reachable with --n 33).
+The state is far larger than the 126 MB L2, so no L2 flush is needed between iterations.
+
+With N > 1 (torchrun) every rank transforms its own state (replicas only: the path does not shard,
+DESIGN.md section "multi-GPU"); value = all ranks' work / max-over-ranks time, "scaling": "weak".
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample
+of the same workload; see DESIGN.md "measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--n", type=int, default=30, help="qubits (state = 2^n complex64)")
+    ap.add_argument("--k", type=int, default=None, help="AQFT cutoff (default: exact)")
+    ap.add_argument("--max-fused", type=int, default=13)
+    ap.add_argument("--tile-bits", type=int, default=0)
+    ap.add_argument("--hub-bits", type=int, default=0)
+    ap.add_argument("--flags", type=int, default=0)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", default="", help="comma list of extra n to time briefly, e.g. 20,22,26,33")
+    return ap.parse_args()
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.lines if t0 - 0.05 <= t <= t1 + 0.15] or [l for (_, l) in self.lines]
+        for l in rows:
+            p = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(p[0]))
+                smax = float(p[1])
+                for nm, v in zip(names, p[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_setup(args):
+    import torch
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return world, rank, local
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.barrier()
+
+
+def max_over_ranks(x: float, world: int, device) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def time_config(qft, torch, n, k, args, steps, warmup, per_pass=True):
+    """Device-resident timing of qft_execute on a fresh synthetic state; returns a dict."""
+    import qft_inputs as qi
+
+    dev = torch.device("cuda", torch.cuda.current_device())
+    plan = qft.Plan(n, n if k is None else k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
+                    args.hub_bits, args.flags)
+    state = torch.empty(1 << n, dtype=torch.complex64, device=dev)
+    if n <= 27:
+        state.copy_(torch.from_numpy(qi.gaussian(n, 1)))
+    else:
+        qi.gaussian_device(n, 2, device=dev, out=state)
+    stream = torch.cuda.current_stream(dev)
+    sptr = stream.cuda_stream
+    for _ in range(warmup):
+        qft.qft_execute(plan.handle, state.data_ptr(), sptr)
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record(stream)
+    for i in range(steps):
+        qft.qft_execute(plan.handle, state.data_ptr(), sptr)
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    total_ms = ev[0].elapsed_time(ev[steps])
+    per_step = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(steps))
+    res = {"plan": plan, "state": state, "total_ms": total_ms, "median_ms": per_step[len(per_step) // 2],
+           "min_ms": per_step[0], "passes": plan.num_passes, "launches": plan.num_launches}
+    if per_pass:
+        # per-pass CUDA-event timing (same stream), cycling through the passes in order so that the
+        # state keeps going through whole transforms
+        npass = plan.num_passes
+        reps = max(3, min(steps, 10))
+        acc = [0.0] * npass
+        for _ in range(reps):
+            evs = [torch.cuda.Event(enable_timing=True) for _ in range(npass + 1)]
+            evs[0].record(stream)
+            for p in range(npass):
+                qft.qft_execute_pass(plan.handle, p, state.data_ptr(), sptr)
+                evs[p + 1].record(stream)
+            torch.cuda.synchronize()
+            for p in range(npass):
+                acc[p] += evs[p].elapsed_time(evs[p + 1])
+        res["pass_ms"] = [a / reps for a in acc]
+    return res
+
+
+def oracle_sample(n, k, reps=1):
+    """Time a bounded sample of the oracle's gate-by-gate circuit on the full 2^n fp64 state and
+    extrapolate to the whole circuit: t = n_H t_H + n_CR t_CR + n_SWAP t_SWAP."""
+    import numpy as np
+
+    import oracle
+
+    gates = oracle.gate_list(n, n if k is None else k)
+    n_h = int((gates[:, 0] == oracle.GATE_H).sum())
+    n_cr = int((gates[:, 0] == oracle.GATE_CR).sum())
+    n_sw = int((gates[:, 0] == oracle.GATE_SWAP).sum())
+    s = np.zeros(1 << n, dtype=np.complex128)
+    s[:] = 1.0 / math.sqrt(1 << n)
+    hs = [g for g in gates if g[0] == oracle.GATE_H]
+    crs = [g for g in gates if g[0] == oracle.GATE_CR]
+    sws = [g for g in gates if g[0] == oracle.GATE_SWAP]
+    sample = [hs[0], hs[-1]] + ([crs[0], crs[len(crs) // 2]] if crs else []) + (sws[:1] if sws else [])
+    t = {0: [], 1: [], 2: []}
+    for _ in range(reps):
+        for g in sample:
+            t0 = time.perf_counter()
+            oracle.apply_gate_inplace(s, g)
+            t[int(g[0])].append(time.perf_counter() - t0)
+    mean = lambda v: sum(v) / len(v) if v else 0.0
+    est = n_h * mean(t[0]) + n_cr * mean(t[1]) + n_sw * mean(t[2])
+    spent = sum(sum(v) for v in t.values())
+    desc = (f"{len(sample)} of the {len(gates)} gates of the n={n} circuit (H q{int(hs[0][1])}, H q{int(hs[-1][1])}, "
+            f"2 CR, 1 SWAP) on the full 2^{n} fp64 state; whole-circuit time extrapolated as "
+            f"n_H*t_H + n_CR*t_CR + n_SWAP*t_SWAP = {est:.1f} s ({spent:.1f} s measured)")
+    return est, spent, desc, oracle.max_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    n = args.n
+    flops = 5.0 * (1 << n) * n
+    # keep the whole run within a few minutes: the per-step sample is ~5 gates on the full state
+    n_eff = n
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    budget_steps = 3
+    steps_run = min(steps, budget_steps)
+    warm_run = min(warmup, 1)
+    vals = []
+    desc = ""
+    cores = 1
+    for i in range(warm_run + steps_run):
+        est, spent, desc, cores = oracle_sample(n_eff, args.k)
+        if i >= warm_run:
+            vals.append(est)
+    est = sorted(vals)[len(vals) // 2]
+    gf = flops / est / 1e9
+    line = {
+        "impl": "reference", "metric": "dft_equiv_gflops", "value": gf, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "steps": steps_run, "warmup": warm_run, "ms_per_step": est * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"n={n} {'exact QFT' if args.k is None else 'AQFT k=%d' % args.k}, "
+                               f"2^{n} amplitudes, CPU oracle (gate-by-gate fp64, OpenMP)"},
+        "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": gf, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+        "note": f"requested steps={steps} warmup={warmup}; ran {steps_run}+{warm_run} bounded samples",
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback for the QFT path)")
+    qft.load()
+    world, rank, local = dist_setup(args)
+    torch.cuda.set_device(local % torch.cuda.device_count())
+    dev = torch.device("cuda", torch.cuda.current_device())
+    n, steps, warmup = args.n, max(1, args.steps), max(3, args.warmup)
+    N = 1 << n
+    flops = 5.0 * N * n
+    peak, peak_src = measured_peak_gbs()
+
+    # ---- device-resident timing: W warm-ups, then exactly K steps between barriers ----
+    import qft_inputs as qi
+
+    plan = qft.Plan(n, n if args.k is None else args.k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
+                    args.hub_bits, args.flags)
+    state = torch.empty(N, dtype=torch.complex64, device=dev)
+    if n <= 27:
+        state.copy_(torch.from_numpy(qi.gaussian(n, 1)))
+    else:
+        qi.gaussian_device(n, 2, device=dev, out=state)
+    stream = torch.cuda.current_stream(dev)
+    sptr = stream.cuda_stream
+    for _ in range(warmup):
+        qft.qft_execute(plan.handle, state.data_ptr(), sptr)
+    torch.cuda.synchronize()
+    barrier(world)
+    sampler = ClockSampler(torch.cuda.current_device())
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record(stream)
+    for _ in range(steps):
+        qft.qft_execute(plan.handle, state.data_ptr(), sptr)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.time()
+    barrier(world)
+    total_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    ms_per_step = total_ms / steps
+    value = world * flops / (ms_per_step * 1e-3) / 1e9
+
+    # ---- per-pass timing for the roofline of the dominant kernel ----
+    npass = plan.num_passes
+    reps = max(3, min(steps, 10))
+    acc = [0.0] * npass
+    for _ in range(reps):
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(npass + 1)]
+        evs[0].record(stream)
+        for p in range(npass):
+            qft.qft_execute_pass(plan.handle, p, state.data_ptr(), sptr)
+            evs[p + 1].record(stream)
+        torch.cuda.synchronize()
+        for p in range(npass):
+            acc[p] += evs[p].elapsed_time(evs[p + 1])
+    pass_ms = [a / reps for a in acc]
+    desc = plan.describe()
+    kernels = [p["kernel"] for p in desc["passes"]]
+    # dominant kernel = the kernel kind with the largest share of the step
+    share = {}
+    for kname, ms in zip(kernels, pass_ms):
+        share.setdefault(kname, []).append(ms)
+    dom = max(share, key=lambda kk: sum(share[kk]))
+    dom_ms = sum(share[dom]) / len(share[dom])
+    bytes_per_launch = 16.0 * N  # 8 B read + 8 B written per amplitude per pass
+    achieved = bytes_per_launch / (dom_ms * 1e-3) / 1e9
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            tj = json.load(fh)
+        ent = tj.get(f"n{n}", {}).get(dom)
+        if ent:
+            traffic = float(ent["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "bytes_per_launch": bytes_per_launch, "launch_ms": dom_ms,
+                "pass_ms": pass_ms, "pass_kernels": kernels,
+                "step_gbs": npass * bytes_per_launch / (ms_per_step * 1e-3) / 1e9,
+                "step_frac": npass * bytes_per_launch / (ms_per_step * 1e-3) / 1e9 / peak}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        try:
+            host = torch.empty(N, dtype=torch.complex64).pin_memory()
+            host.copy_(state.cpu() if n <= 27 else state.to("cpu", non_blocking=False))
+            e2e_steps = max(1, min(steps, 3 if n >= 28 else 10))
+            qft.qft_execute_host(plan.handle, host.data_ptr(), sptr)  # warm-up (allocates the plan's device buffer)
+            torch.cuda.synchronize()
+            barrier(world)
+            ta = time.perf_counter()
+            for _ in range(e2e_steps):
+                qft.qft_execute_host(plan.handle, host.data_ptr(), sptr)
+            torch.cuda.synchronize()
+            tb = time.perf_counter()
+            e2e_ms = max_over_ranks((tb - ta) * 1e3 / e2e_steps, world, dev)
+            e2e = {"value": world * flops / (e2e_ms * 1e-3) / 1e9, "unit": "GFLOP/s", "h2d_bytes_per_step": 8 * N,
+                   "d2h_bytes_per_step": 8 * N, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                   "host_memory": "pinned"}
+            del host
+        except Exception as exc:  # e.g. not enough pinned host memory
+            e2e = {"value": None, "unit": "GFLOP/s", "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 8 * N,
+                   "error": str(exc)}
+
+    # ---- optional brief sweep over other n (reported, not the headline) ----
+    sweep = []
+    if args.sweep and rank == 0:
+        del state
+        plan.close()
+        torch.cuda.empty_cache()
+        for sn in [int(v) for v in args.sweep.split(",") if v]:
+            st = 5 if sn >= 32 else 10
+            r = time_config(qft, torch, sn, None, args, st, 3, per_pass=True)
+            sweep.append({"n": sn, "passes": r["passes"], "median_ms": r["median_ms"],
+                          "gflops": 5.0 * (1 << sn) * sn / (r["median_ms"] * 1e-3) / 1e9,
+                          "gbs": r["passes"] * 16.0 * (1 << sn) / (r["median_ms"] * 1e-3) / 1e9,
+                          "pass_ms": r["pass_ms"]})
+            r["plan"].close()
+            del r
+            torch.cuda.empty_cache()
+
+    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N = 1 only ----
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        try:
+            torch.cuda.empty_cache()
+            est, spent, sdesc, cores = oracle_sample(n, args.k)
+            cpu_baseline = {"value": flops / est / 1e9, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
+                            "sample": sdesc, "seconds_estimated": est}
+        except Exception as exc:
+            cpu_baseline = {"value": None, "unit": "GFLOP/s", "cores": os.cpu_count(), "kind": "oracle",
+                            "sample": f"failed: {exc}"}
+
+    if rank == 0:
+        line = {
+            "metric": "dft_equiv_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": steps,
+            "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"n={n} {'exact QFT' if args.k is None else 'AQFT k=%d' % args.k}: "
+                                   f"2^{n} complex64 amplitudes ({8 * N / 2 ** 30:.3g} GiB) per GPU, in place, "
+                                   f"forward sign, unitary scaling, natural order in and out",
+                       "n_qubits": n, "aqft_cutoff_k": desc["k"], "passes": npass, "ideal_passes": math.ceil(n / 13),
+                       "tile_bits": desc["tile_bits"], "hub_bits": desc["hub_bits"], "folded_bit_reversal": desc["folded"],
+                       "l2": "state larger than L2, no flush needed" if 8 * N > 2 * 126e6 else
+                             "state fits L2: HBM fraction not meaningful",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "time_ms": ms_per_step, "hbm_gbs": roofline["step_gbs"], "hbm_frac_of_measured_peak": roofline["step_frac"],
+            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline, "gpu_launches": steps * plan.num_launches
+            if not sweep else steps * npass,
+            "clocks": clocks,
+        }
+        if sweep:
+            line["sweep"] = sweep
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -117,6 +117,13 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
  */
 qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream);
 
+/*
+ * qft_execute_pass -- enqueue only pass `pass_index` (0 .. qft_plan_num_passes-1) of the plan.
+ * Running every pass in order is exactly qft_execute; a single pass is a profiling aid (per-pass
+ * CUDA-event timing for the roofline report) and leaves the state in an intermediate layout.
+ */
+qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_state, void* stream);
+
 /* qft_plan_destroy -- free the plan and everything it owns.  NULL is allowed. */
 qft_status_t qft_plan_destroy(qft_plan_t plan);
 

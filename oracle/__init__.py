@@ -113,6 +113,20 @@ def apply_swap(x, a: int, b: int) -> np.ndarray:
     return s
 
 
+def apply_gate_inplace(s: np.ndarray, gate, sign: int = -1) -> None:
+    """One gate {type, q0, q1, m} on a complex128 state, in place (used to time a bounded
+    sample of a circuit that is too long to run whole)."""
+    assert s.dtype == np.complex128 and s.flags.c_contiguous
+    n = _n_of(s)
+    ty, q0, q1, m = (int(v) for v in gate)
+    if ty == GATE_H:
+        lib().orc_apply_h(_dp(s), n, q0)
+    elif ty == GATE_CR:
+        lib().orc_apply_cr(_dp(s), n, q0, q1, m, sign)
+    else:
+        lib().orc_apply_swap(_dp(s), n, q0, q1)
+
+
 def run_gates(x, gates: np.ndarray, sign: int = -1) -> np.ndarray:
     s = _state(x)
     g = np.ascontiguousarray(gates, dtype=np.int32)

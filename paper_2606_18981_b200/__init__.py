@@ -25,7 +25,7 @@ QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED = 1, 2
 QFT_MAX_QUBITS = 34
 
 EXPORTS = [
-    "qft_plan_create", "qft_plan_create_tuned", "qft_execute", "qft_execute_host", "qft_plan_destroy",
+    "qft_plan_create", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
     "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
 ]
@@ -63,6 +63,8 @@ def load() -> ctypes.CDLL:
     L.qft_plan_create_tuned.restype = ci
     L.qft_execute.argtypes = [vp, vp, vp]
     L.qft_execute.restype = ci
+    L.qft_execute_pass.argtypes = [vp, ci, vp, vp]
+    L.qft_execute_pass.restype = ci
     L.qft_execute_host.argtypes = [vp, vp, vp]
     L.qft_execute_host.restype = ci
     L.qft_plan_destroy.argtypes = [vp]
@@ -120,6 +122,12 @@ def qft_execute(plan: int, device_state_ptr: int, stream: int = 0) -> None:
     st = load().qft_execute(plan, device_state_ptr, stream)
     if st != QFT_OK:
         raise QftError(st, "qft_execute")
+
+
+def qft_execute_pass(plan: int, pass_index: int, device_state_ptr: int, stream: int = 0) -> None:
+    st = load().qft_execute_pass(plan, pass_index, device_state_ptr, stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_execute_pass")
 
 
 def qft_execute_host(plan: int, host_state_ptr: int, stream: int = 0) -> None:

@@ -75,6 +75,15 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream) {
     return QFT_OK;
 }
 
+qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_state, void* stream) {
+    if (!plan || !device_state || pass_index < 0 || pass_index >= (int)plan->host.passes.size())
+        return QFT_ERR_INVALID_ARG;
+    if (((uintptr_t)device_state) & 15) return QFT_ERR_INVALID_ARG;
+    cudaError_t e = qft_launch_pass(plan->host.passes[pass_index], device_state, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return QFT_OK;
+}
+
 qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream) {
     if (!plan || !host_state) return QFT_ERR_INVALID_ARG;
     const size_t bytes = (size_t)8 << plan->host.prm.n;

@@ -1,0 +1,112 @@
+"""Checkers for states too large for the CPU oracle (n = 30, 33): test infrastructure only.
+
+Everything here is float64 torch arithmetic that runs on whatever device holds the state (the
+8-64 GiB inputs live in HBM), written from closed forms that tests/test_oracle_pins.py and
+tests/test_large_checks_cpu.py pin against the gate-by-gate oracle at small n on the CPU:
+
+  sampled_outputs()      out[K] = 2^{-n/2} sum_j x[j] exp(2 pi i turns_k(K, j)), the circuit's matrix
+                         element (oracle.orc_element_turns) summed over the whole input:
+                         turns_k(K, j) = sign * sum_{t : y_t = 1} tr_{k,t}(j) / 2^{t+1},
+                         y_t = bit n-1-t of K, tr_{k,t}(j) = (j mod 2^{t+1}) with bits below t-k
+                         cleared.  For k >= n-1 this is the DFT phase sign * (j K mod N) / N.
+  tones_closed_form()    AQFT_k of a sum of tones, every output, by factorising over input bits:
+                         out[K] = sum_i a_i prod_c (1 + exp(2 pi i alpha_c)) / 2,
+                         alpha_c = f_i 2^c / N - field_c(K) / 2^{k+1}.
+  norm2()                float64 sum of |x|^2 (Parseval).
+None of this is used by the product path.
+"""
+from __future__ import annotations
+
+import math
+
+import torch
+
+
+def _chunks(n, chunk_bits):
+    cb = min(chunk_bits, n)
+    return cb, 1 << cb, 1 << (n - cb)
+
+
+def norm2(x: torch.Tensor, chunk_bits: int = 26) -> float:
+    v = torch.view_as_real(x)
+    n = int(x.numel()).bit_length() - 1
+    cb, C, nc = _chunks(n, chunk_bits)
+    acc = torch.zeros((), dtype=torch.float64, device=x.device)
+    for c in range(nc):
+        blk = v[c * C:(c + 1) * C].to(torch.float64)
+        acc += (blk * blk).sum()
+    return float(acc.item())
+
+
+def sampled_outputs(x: torch.Tensor, Ks, k: int, sign: int = -1, chunk_bits: int = 24) -> torch.Tensor:
+    """Direct float64 sums for the output indices Ks (unitary scaling); x is the INPUT state."""
+    N = x.numel()
+    n = int(N).bit_length() - 1
+    cb, C, nc = _chunks(n, chunk_bits)
+    dev = x.device
+    base = torch.arange(C, dtype=torch.int64, device=dev)
+    out = torch.zeros(len(Ks), dtype=torch.complex128, device=dev)
+    exact = k >= n - 1
+    for c in range(nc):
+        j = base + c * C
+        xc = x[c * C:(c + 1) * C].to(torch.complex128)
+        for s, K in enumerate(Ks):
+            K = int(K)
+            if exact:
+                p = (j * K) & (N - 1)  # int64 wrap-around is exact modulo 2^n
+                turns = p.to(torch.float64) * (float(sign) / N)
+            else:
+                turns = torch.zeros(C, dtype=torch.float64, device=dev)
+                for t in range(n):
+                    if not (K >> (n - 1 - t)) & 1:
+                        continue
+                    tr = j & ((1 << (t + 1)) - 1)
+                    if t - k > 0:
+                        tr = tr & ~((1 << (t - k)) - 1)
+                    turns += tr.to(torch.float64) * (float(sign) / float(1 << (t + 1)))
+            ang = turns * (2.0 * math.pi)
+            w = torch.complex(torch.cos(ang), torch.sin(ang))
+            out[s] += (xc * w).sum()
+    return out * (2.0 ** (-0.5 * n))
+
+
+def tones_closed_form_chunk(n: int, k: int, freqs, phases, K: torch.Tensor) -> torch.Tensor:
+    """AQFT_k (forward sign, unitary) of the multi_tone() input at the output indices K (int64)."""
+    N = 1 << n
+    dev = K.device
+    amp = 1.0 / math.sqrt(len(freqs))
+    acc = torch.zeros(K.shape, dtype=torch.complex128, device=dev)
+    kk = min(k, n - 1)
+    for f, th in zip(freqs, phases):
+        f = int(f)
+        re = torch.full(K.shape, math.cos(float(th)) * amp, dtype=torch.float64, device=dev)
+        im = torch.full(K.shape, math.sin(float(th)) * amp, dtype=torch.float64, device=dev)
+        for c in range(n):
+            top = min(n - 1, c + kk)           # highest target t that sees bit c as a control (or itself)
+            width = top - c + 1                 # bits y_c .. y_top = bits n-1-c .. n-1-top of K
+            field = (K >> (n - 1 - top)) & ((1 << width) - 1)
+            # sum_{t=c..top} y_t 2^{c-t-1}: y_c is the field's most significant bit, weight 1/2
+            al = (((f << c) % N) / N) - field.to(torch.float64) * (1.0 / float(1 << width))
+            ang = al * (2.0 * math.pi)
+            fr = 0.5 * (1.0 + torch.cos(ang))
+            fi = 0.5 * torch.sin(ang)
+            re, im = re * fr - im * fi, re * fi + im * fr
+        acc += torch.complex(re, im)
+    return acc
+
+
+def tones_rel_l2(y: torch.Tensor, n: int, k: int, freqs, phases, chunk_bits: int = 22, index_chunks=None):
+    """Relative L2 distance between the device result y and the closed form, over all outputs or
+    over the listed chunks of 2^chunk_bits consecutive outputs.  Returns (rel_l2, ref_norm2)."""
+    cb, C, nc = _chunks(n, chunk_bits)
+    dev = y.device
+    base = torch.arange(C, dtype=torch.int64, device=dev)
+    num = torch.zeros((), dtype=torch.float64, device=dev)
+    den = torch.zeros((), dtype=torch.float64, device=dev)
+    for c in (range(nc) if index_chunks is None else index_chunks):
+        K = base + c * C
+        ref = tones_closed_form_chunk(n, k, freqs, phases, K)
+        d = y[c * C:(c + 1) * C].to(torch.complex128) - ref
+        num += (d.real * d.real + d.imag * d.imag).sum()
+        den += (ref.real * ref.real + ref.imag * ref.imag).sum()
+    return math.sqrt(float(num.item()) / float(den.item())), float(den.item())

@@ -184,6 +184,14 @@ __device__ __forceinline__ void decode_tile(uint32_t bid, int p, uint32_t* mload
     *mstore = y | (x << p) | (z << (2 * p));
 }
 
+// Streaming 8-byte global load: every amplitude is read exactly once per pass, so do not allocate
+// in L1.  (Plain ld.global, not the non-coherent path: the same kernel later writes these addresses.)
+__device__ __forceinline__ float2 ld_stream(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 

@@ -15,6 +15,7 @@
 #include <stdint.h>
 
 #include "qft_device.cuh"
+#include "qft_fused.cuh"
 #include "qft_plan.h"
 
 namespace qftk {
@@ -152,24 +153,43 @@ __global__ void __launch_bounds__(256) qft_tile_pass_generic(float2* __restrict_
 // ---------------------------------------------------------------------------------------------
 // launcher
 // ---------------------------------------------------------------------------------------------
-static cudaError_t ensure_attrs() {
-    static bool done = false;
-    static cudaError_t st = cudaSuccess;
-    if (!done) {
-        st = cudaFuncSetAttribute(qftk::qft_tile_pass_generic, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  8 << QFT_MAX_TILE_BITS);
-        if (st == cudaSuccess) done = true;
+typedef void (*pass_kernel_t)(float2*, const QftPassDesc);
+
+static pass_kernel_t pick_kernel(const QftPassDesc& d) {
+    if (d.kernel == QFT_KERNEL_FUSED2) {
+        const int r1 = d.steps[0].r, r2 = d.steps[1].r;
+        const bool fast = d.k >= 4;  // no in-group truncation for any radix <= 32
+#define QFT_PICK(A, B)                                                                   \
+    if (r1 == A && r2 == B)                                                              \
+        return fast ? (pass_kernel_t)qftk::qft_pass_fused2<A, B, true> : (pass_kernel_t)qftk::qft_pass_fused2<A, B, false>;
+        QFT_PICK(5, 5)
+        QFT_PICK(5, 4)
+        QFT_PICK(4, 4)
+        QFT_PICK(4, 3)
+        QFT_PICK(3, 3)
+#undef QFT_PICK
     }
-    return st;
+    return (pass_kernel_t)qftk::qft_tile_pass_generic;
+}
+
+bool qft_fused2_supported(int r1, int r2) {
+    return (r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3) ||
+           (r1 == 3 && r2 == 3);
 }
 
 cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream) {
-    cudaError_t e = ensure_attrs();
-    if (e != cudaSuccess) return e;
+    pass_kernel_t kern = pick_kernel(d);
+    const size_t smem = (size_t)8 << d.f;
+    if (smem > 48 * 1024) {
+        // idempotent and cheap; needed once per kernel instantiation
+        cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             8 << QFT_MAX_TILE_BITS);
+        if (e != cudaSuccess) return e;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(1u << d.ntile);
     cfg.blockDim = dim3(1u << d.log2_threads);
-    cfg.dynamicSmemBytes = (size_t)8 << d.f;
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     cfg.attrs = attr;
@@ -181,5 +201,6 @@ cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stre
         attr[0].val.clusterDim.z = 1;
         cfg.numAttrs = 1;
     }
-    return cudaLaunchKernelEx(&cfg, qftk::qft_tile_pass_generic, (float2*)state, d);
+    void* args[2] = {(void*)&state, (void*)&d};
+    return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
 }

@@ -147,8 +147,8 @@ std::vector<int> step_sizes(int w) {
 }
 
 // Turn a PassSpec into the kernel descriptor given the current layout; updates qubit_at.
-bool lower_pass(const PassSpec& ps, int n, int k, int conj, std::vector<int>& qubit_at, QftPassDesc* d,
-                std::string* err) {
+bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, std::vector<int>& qubit_at,
+                QftPassDesc* d, std::string* err) {
     std::memset(d, 0, sizeof(*d));
     const int f = (int)ps.F.size();
     if (f > QFT_MAX_TILE_BITS || n - f > QFT_MAX_TILEIDX_BITS) { *err = "tile too large"; return false; }
@@ -221,6 +221,66 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, std::vector<int>& qu
             t -= r;
         }
     }
+    // fused two-step kernel: eligible when the hub's qubits are not in the register group of the
+    // step that touches HBM (so that the lanes of a warp can walk whole granules)
+    if (d->nsteps == 2 && allow_fused) {
+        const QftStep s1 = d->steps[0], s2 = d->steps[1];
+        auto in_group = [](const QftStep& s, int c) { return c >= s.a && c < s.a + s.r; };
+        const int l = std::min(hub, f);
+        bool ok = true;
+        for (int j = 0; j < l; ++j) {
+            if (in_group(s1, d->ld_canon[j])) ok = false;
+            if (in_group(s2, d->st_canon[j])) ok = false;
+        }
+        if (f - std::max<int>(s1.r, s2.r) < 5) ok = false;  // at least one warp of butterflies
+        if (ok) {
+            d->kernel = QFT_KERNEL_FUSED2;
+            int lt2 = f - std::max<int>(s1.r, s2.r);
+            d->log2_threads = std::min(lt2, 8);
+            std::vector<int> addr_of_canon_ld(f), addr_of_canon_st(f);
+            for (int j = 0; j < f; ++j) {
+                addr_of_canon_ld[d->ld_canon[j]] = d->F[j];
+                addr_of_canon_st[d->st_canon[j]] = d->F[j];
+            }
+            int nt = 0;
+            for (int j = 0; j < f; ++j)
+                if (!in_group(s1, d->ld_canon[j])) { d->t1_addr[nt] = d->F[j]; d->t1_canon[nt] = d->ld_canon[j]; ++nt; }
+            for (int b = 0; b < s1.r; ++b) d->r1_addr[b] = (int8_t)addr_of_canon_ld[s1.a + b];
+            nt = 0;
+            for (int j = 0; j < f; ++j)
+                if (!in_group(s2, d->st_canon[j])) { d->t2_addr[nt] = d->F[j]; d->t2_canon[nt] = d->st_canon[j]; ++nt; }
+            for (int b = 0; b < s2.r; ++b) d->r2_addr[b] = (int8_t)addr_of_canon_st[s2.a + b];
+            // swizzle: canonical bits 0..3 keep their own bank bit; the four lowest lane bits of each
+            // step (a half-warp = one 128-byte shared-memory wavefront of 8-byte accesses) must get
+            // linearly independent masks
+            for (int c = 0; c < 16; ++c) d->swz_col[c] = 0;
+            for (int c = 0; c < std::min(4, f); ++c) d->swz_col[c] = (uint8_t)(1u << c);
+            auto fix = [&](const int8_t* lane_canon, int nl) {
+                // span of the masks already fixed among these lanes
+                std::vector<int> vecs;
+                for (int i = 0; i < nl; ++i)
+                    if (d->swz_col[lane_canon[i]]) vecs.push_back(d->swz_col[lane_canon[i]]);
+                auto span = [&](const std::vector<int>& vs) {
+                    std::set<int> sp{0};
+                    for (int v : vs) {
+                        std::set<int> add;
+                        for (int x : sp) add.insert(x ^ v);
+                        sp.insert(add.begin(), add.end());
+                    }
+                    return sp;
+                };
+                for (int i = 0; i < nl; ++i) {
+                    const int c = lane_canon[i];
+                    if (d->swz_col[c]) continue;
+                    std::set<int> sp = span(vecs);
+                    for (int v = 1; v < 16; ++v)
+                        if (!sp.count(v)) { d->swz_col[c] = (uint8_t)v; vecs.push_back(v); break; }
+                }
+            };
+            fix(d->t1_canon, std::min(4, f - s1.r));
+            fix(d->t2_canon, std::min(4, f - s2.r));
+        }
+    }
     // apply the permutation to the tracking
     std::vector<int> nq(qubit_at);
     for (int a : ps.F) nq[dest[a]] = qubit_at[a];
@@ -268,7 +328,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     int wmaxseen = 0;
     for (auto& ps : specs) {
         QftPassDesc d;
-        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, qubit_at, &d, err)) return 5;
+        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), qubit_at, &d, err)) return 5;
         wmaxseen = std::max(wmaxseen, (int)ps.window.size());
         out->passes.push_back(d);
     }

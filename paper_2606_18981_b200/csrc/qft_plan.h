@@ -56,6 +56,16 @@ struct QftPassDesc {
     int8_t tile_addr[QFT_MAX_TILEIDX_BITS];  // tile-index bit -> address bit
     int8_t log_tile[QFT_MAX_TILEIDX_BITS];   // tile-index bit -> logical qubit held at load time
     QftStep steps[QFT_MAX_STEPS];
+    // ---- QFT_KERNEL_FUSED2 only -------------------------------------------------------------
+    // Step 1 reads its 2^r1 amplitudes straight from HBM, step 2 writes its 2^r2 straight back.
+    // t?_addr / t?_canon: for every bit of the thread's "other" index (load order for step 1, store
+    // order for step 2, the step's own bits left out) the address bit and the canonical bit.
+    // r?_addr: address bit of the step's b-th register bit (canonical bit a + b).
+    // swz_col[c]: 4-bit XOR mask that canonical bit c contributes to the low 4 bits of the
+    // shared-memory index (a GF(2)-linear, conflict-free swizzle chosen by the planner).
+    int8_t t1_addr[16], t1_canon[16], r1_addr[QFT_MAX_RADIX_BITS + 3];
+    int8_t t2_addr[16], t2_canon[16], r2_addr[QFT_MAX_RADIX_BITS + 3];
+    uint8_t swz_col[16];
 };
 
 #include <string>

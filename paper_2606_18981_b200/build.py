@@ -11,8 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqft.so")
-SOURCES = ["qft_api.cu", "qft_kernels.cu", "qft_plan.cpp"]
-HEADERS = ["qft_plan.h", "qft_device.cuh", os.path.join("..", "..", "include", "qft.h")]
+SOURCES = ["qft_api.cu", "qft_kernels.cu", "qft_tma_lt7.cu", "qft_tma_lt8.cu", "qft_tma_lt9.cu", "qft_plan.cpp"]
+HEADERS = ["qft_plan.h", "qft_device.cuh", "qft_fused.cuh", "qft_tma.cuh", "qft_tma_inst.cuh", "qft_packed.cuh", os.path.join("..", "..", "include", "qft.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
@@ -33,11 +33,25 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile every source to an object file in parallel (one nvcc process each), then link."""
     if force or _stale():
+        from concurrent.futures import ThreadPoolExecutor
+
         nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
-              [os.path.join(CSRC, s) for s in SOURCES]
-        subprocess.run(cmd, check=True)
+        objdir = os.path.join(HERE, "build")
+        os.makedirs(objdir, exist_ok=True)
+        cflags = [f for f in NVCC_FLAGS if f not in ("-shared",)]
+
+        def compile_one(src: str) -> str:
+            obj = os.path.join(objdir, os.path.splitext(src)[0] + ".o")
+            cmd = [nvcc] + cflags + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+            subprocess.run(cmd, check=True)
+            return obj
+
+        with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+            objs = list(ex.map(compile_one, SOURCES))
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static",
+                        "-o", LIB] + objs, check=True)
     return LIB
 
 

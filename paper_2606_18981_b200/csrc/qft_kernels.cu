@@ -16,6 +16,7 @@
 
 #include "qft_device.cuh"
 #include "qft_fused.cuh"
+#include <cuda.h>
 #include "qft_plan.h"
 
 namespace qftk {
@@ -177,7 +178,97 @@ bool qft_fused2_supported(int r1, int r2) {
            (r1 == 3 && r2 == 3);
 }
 
+// ---- QFT_KERNEL_TMA2 ---------------------------------------------------------------------------
+typedef void (*tma2_kernel_t)(float2*, const CUtensorMap, const QftPassDesc);
+tma2_kernel_t qft_pick_tma2_lt7(int r1, int r2, int kc);  // qft_tma_lt7.cu
+tma2_kernel_t qft_pick_tma2_lt8(int r1, int r2, int kc);  // qft_tma_lt8.cu
+tma2_kernel_t qft_pick_tma2_lt9(int r1, int r2, int kc);  // qft_tma_lt9.cu
+
+static tma2_kernel_t pick_tma2(const QftPassDesc& d) {
+    const int kc = d.k < 4 ? d.k : 4;
+    switch (d.log2_threads) {
+        case 7: return qft_pick_tma2_lt7(d.tma.r1, d.tma.r2, kc);
+        case 8: return qft_pick_tma2_lt8(d.tma.r1, d.tma.r2, kc);
+        case 9: return qft_pick_tma2_lt9(d.tma.r1, d.tma.r2, kc);
+    }
+    return nullptr;
+}
+
+typedef CUresult (*encode_tiled_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static encode_tiled_t get_encode_tiled() {
+    static encode_tiled_t fn = []() -> encode_tiled_t {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess)
+            return nullptr;
+        return (encode_tiled_t)p;
+    }();
+    return fn;
+}
+
+static int sm_count() {
+    static int n = []() {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) return 148;
+        return v;
+    }();
+    return n;
+}
+
+int g_qft_tma_l2promo = 1;  // CUtensorMapL2promotion: 0 none, 1 64 B, 2 128 B, 3 256 B (tuning knob)
+
+static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t stream) {
+    tma2_kernel_t kern = pick_tma2(d);
+    encode_tiled_t enc = get_encode_tiled();
+    if (!kern || !enc) return cudaErrorNotSupported;
+    CUtensorMap map;
+    cuuint64_t gdim[5], gstr[4];
+    cuuint32_t box[5], estr[5];
+    for (int i = 0; i < 5; ++i) {
+        gdim[i] = 1ull << d.tma.tma_len[i];
+        box[i] = 1u << d.tma.tma_box[i];
+        estr[i] = 1;
+        if (i > 0) gstr[i - 1] = 8ull << d.tma.tma_lo[i];
+    }
+    CUresult r = enc(&map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 5, state, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, (CUtensorMapL2promotion)g_qft_tma_l2promo,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES;
+    cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int per_sm = d.f == 13 ? 2 : (d.f == 12 ? 4 : 1);
+    const unsigned csz = d.npair ? 2u : 1u;
+    unsigned long long ntiles = 1ull << d.ntile;
+    unsigned long long grid = (unsigned long long)sm_count() * per_sm;
+    if (grid > ntiles) grid = ntiles;
+    grid -= grid % csz;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(1u << d.log2_threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    cfg.attrs = attr;
+    cfg.numAttrs = 0;
+    if (d.npair > 0) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.numAttrs = 1;
+    }
+    void* args[3] = {(void*)&state, (void*)&map, (void*)&d};
+    return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
+}
+
 cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream) {
+    if (d.kernel == QFT_KERNEL_TMA2) return launch_tma2(d, state, stream);
     pass_kernel_t kern = pick_kernel(d);
     const size_t smem = (size_t)8 << d.f;
     if (smem > 48 * 1024) {

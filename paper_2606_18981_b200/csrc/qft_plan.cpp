@@ -146,9 +146,206 @@ std::vector<int> step_sizes(int w) {
     return split_balanced(w, g);  // larger groups first
 }
 
+
+// ---- QFT_KERNEL_TMA2 lowering -----------------------------------------------------------------
+// Choose 4-bit XOR masks for the canonical bits >= 4 such that the four lowest lane bits of step 1's
+// writers and of step 2's readers each map to linearly independent bank masks (8-byte accesses are
+// served per half-warp: 16 lanes x 8 B = the 32 banks).  Canonical bits < 4 keep their own bank bit.
+// Backtracking over the (at most eight) bits involved.
+bool independent4(const int (&m)[4]) {
+    // Gaussian elimination over GF(2) on four 4-bit vectors
+    int v[4] = {m[0], m[1], m[2], m[3]};
+    int rank = 0;
+    for (int bit = 0; bit < 4; ++bit) {
+        int piv = -1;
+        for (int i = rank; i < 4; ++i)
+            if ((v[i] >> bit) & 1) { piv = i; break; }
+        if (piv < 0) continue;
+        std::swap(v[rank], v[piv]);
+        for (int i = 0; i < 4; ++i)
+            if (i != rank && ((v[i] >> bit) & 1)) v[i] ^= v[rank];
+        ++rank;
+    }
+    return rank == 4;
+}
+
+bool solve_swizzle(const int (&L1)[4], const int (&L2)[4], int f, uint8_t (&lowmask)[16]) {
+    // lowmask[c] = the low-4-bit mask canonical bit c contributes (for c < 4: 1 << c, fixed)
+    for (int c = 0; c < 16; ++c) lowmask[c] = (c < 4) ? (uint8_t)(1u << c) : 0;
+    std::vector<int> freebits;
+    for (int i = 0; i < 4; ++i) {
+        for (int c : {L1[i], L2[i]})
+            if (c >= 4 && std::find(freebits.begin(), freebits.end(), c) == freebits.end()) freebits.push_back(c);
+    }
+    (void)f;
+    auto ok = [&]() {
+        int a[4], b[4];
+        for (int i = 0; i < 4; ++i) { a[i] = lowmask[L1[i]]; b[i] = lowmask[L2[i]]; }
+        return independent4(a) && independent4(b);
+    };
+    // depth-first over assignments (16 choices per free bit, <= 8 bits, pruned only at the leaves: the
+    // search space is at most 16^8 but a solution is found within the first few thousand leaves)
+    std::vector<int> choice(freebits.size(), 0);
+    size_t nfree = freebits.size();
+    if (nfree == 0) return ok();
+    long long budget = 20000000;
+    std::vector<int> idx(nfree, 1);
+    while (budget-- > 0) {
+        for (size_t i = 0; i < nfree; ++i) lowmask[freebits[i]] = (uint8_t)idx[i];
+        if (ok()) return true;
+        size_t i = 0;
+        while (i < nfree) {
+            if (++idx[i] < 16) break;
+            idx[i] = 1;
+            ++i;
+        }
+        if (i == nfree) break;
+    }
+    return false;
+}
+
+// Fills d->tma and sets d->kernel = QFT_KERNEL_TMA2 when the pass fits the kernel's shape.
+void lower_tma2(QftPassDesc* d, int n, int hub) {
+    const int f = d->f;
+    const QftStep s1 = d->steps[0], s2 = d->steps[1];
+    const int r1 = s1.r, r2 = s2.r;
+    if (f < 12 || f > 14) return;
+    if (!((r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3))) return;
+    if (s1.a != s2.a + r2) return;  // the window is one run of canonical bits
+    const int eb = s2.a;            // canonical bits below the window
+    if (eb > 4) return;
+    if (n - f < 1) return;
+    (void)hub;
+    QftTma2Desc t;
+    std::memset(&t, 0, sizeof t);
+    const int lt = f - 5;
+    auto in1 = [&](int c) { return c >= s1.a && c < s1.a + r1; };
+    auto in2 = [&](int c) { return c >= s2.a && c < s2.a + r2; };
+    std::vector<int> inF(n, 0), canon_at_load(n, -1), st_idx_of_canon(f);
+    for (int j = 0; j < f; ++j) {
+        inF[d->F[j]] = 1;
+        canon_at_load[d->F[j]] = d->ld_canon[j];
+        st_idx_of_canon[d->st_canon[j]] = j;
+    }
+    if (!inF[0] || !inF[1]) return;  // the innermost box dimension must span >= 16 bytes
+    // ---- tensor-map dims: runs of address bits inside / outside F.  In-tile runs are cut where the
+    // group membership changes and to <= 8 bits (box <= 256); the run that starts at address bit 0 is
+    // dimension 0 (TMA's contiguous one).  The box lands in shared memory dimension by dimension, so
+    // the order of the other in-tile dims is free: group 1's go last, which keeps its qubits out of
+    // the four lowest landing-index bits (conflict-free reads by lanes that run along the low bits).
+    struct Dim { int lo, len, box, cls; };
+    std::vector<Dim> dims;
+    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return in1(c) ? 2 : (in2(c) ? 1 : 0); };
+    int a = 0;
+    while (a < n) {
+        int b = a + 1;
+        if (inF[a]) {
+            // dimension 0 may mix classes (it is the hub); the others may not
+            while (b < n && inF[b] && b - a < 8 && (cls_of(b) == cls_of(a))) ++b;
+            dims.push_back({a, b - a, b - a, cls_of(a)});
+        } else {
+            while (b < n && !inF[b] && b - a < 30) ++b;
+            dims.push_back({a, b - a, 0, -1});
+        }
+        a = b;
+    }
+    if (dims.size() > 5 || dims[0].box < 1 || dims[0].cls == 2) return;
+    std::stable_sort(dims.begin() + 1, dims.end(), [](const Dim& x, const Dim& y) {
+        const int kx = x.cls == 2 ? 1 : 0, ky = y.cls == 2 ? 1 : 0;
+        return kx < ky;
+    });
+    while (dims.size() < 5) dims.push_back({n, 0, 0, -1});  // size-1 padding dims
+    int nland = 0;
+    std::vector<int> land_idx_of_canon(f, -1);
+    for (int i = 0; i < 5; ++i) {
+        t.tma_lo[i] = (int8_t)dims[i].lo;
+        t.tma_len[i] = (int8_t)dims[i].len;
+        t.tma_box[i] = (int8_t)dims[i].box;
+        for (int b = 0; b < dims[i].box; ++b) {
+            t.land_addr[nland] = (int8_t)(dims[i].lo + b);
+            land_idx_of_canon[canon_at_load[dims[i].lo + b]] = nland;
+            ++nland;
+        }
+    }
+    if (nland != f) return;
+    // ---- threads and registers of the two steps (canonical bits) ----
+    // step 1: register bits = group 1 (+ batch bits: the highest landing bits outside the group);
+    // thread bits = the remaining landing bits, ascending, so lanes read consecutive shared memory
+    std::vector<int> reg1, thr1, reg2, thr2;
+    for (int b = 0; b < r1; ++b) reg1.push_back(s1.a + b);
+    {
+        std::vector<int> rest;
+        for (int j = 0; j < f; ++j) {
+            const int c = canon_at_load[t.land_addr[j]];
+            if (!in1(c)) rest.push_back(c);
+        }
+        while ((int)reg1.size() < 5) { reg1.push_back(rest.back()); rest.pop_back(); }
+        thr1 = rest;
+    }
+    // step 2: register bits = group 2 (+ batch bits); thread bits = the remaining store-order bits,
+    // ascending, so lanes run along the hub and every warp store covers whole granules
+    for (int b = 0; b < r2; ++b) reg2.push_back(s2.a + b);
+    {
+        std::vector<int> rest;
+        for (int j = 0; j < f; ++j)
+            if (!in2(d->st_canon[j])) rest.push_back(d->st_canon[j]);
+        while ((int)reg2.size() < 5) { reg2.push_back(rest.back()); rest.pop_back(); }
+        thr2 = rest;
+    }
+    if ((int)thr1.size() != lt || (int)thr2.size() != lt) return;
+    for (int j = 0; j < 4; ++j)
+        if (land_idx_of_canon[thr1[j]] != j) return;
+    const int hubrun = dims[0].box;
+    for (int j = 0; j < std::min(hubrun, 4); ++j)
+        if (st_idx_of_canon[thr2[j]] != j) return;
+    int L1[4], L2[4];
+    for (int j = 0; j < 4; ++j) { L1[j] = thr1[j]; L2[j] = thr2[j]; }
+    uint8_t lowmask[16];
+    if (!solve_swizzle(L1, L2, f, lowmask)) return;
+    auto midcol = [&](int c) -> uint32_t {
+        const uint32_t slot = (c < 4) ? (1u << c) : ((1u << c) ^ lowmask[c]);
+        return slot << 3;
+    };
+    auto key1 = [&](int c) -> uint16_t {
+        if (in2(c)) return (uint16_t)(1u << (c - s2.a));
+        if (c < eb) return (uint16_t)(1u << (8 + c));
+        return 0;
+    };
+    auto key2 = [&](int c) -> uint16_t {
+        if (in1(c)) return (uint16_t)(1u << (c - s1.a));
+        if (c < eb) return (uint16_t)(1u << (8 + c));
+        return 0;
+    };
+    for (int j = 0; j < lt; ++j) {
+        t.s1_tid_ld[j] = 8u << land_idx_of_canon[thr1[j]];
+        t.s1_tid_mid[j] = midcol(thr1[j]);
+        t.s1_tid_key[j] = key1(thr1[j]);
+        t.s2_tid_mid[j] = midcol(thr2[j]);
+        t.s2_tid_key[j] = key2(thr2[j]);
+        t.s2_tid_addr[j] = d->F[st_idx_of_canon[thr2[j]]];
+    }
+    for (int b = 0; b < 5; ++b) {
+        t.s1_reg_ld[b] = 8u << land_idx_of_canon[reg1[b]];
+        t.s1_reg_mid[b] = midcol(reg1[b]);
+        t.s1_reg_key[b] = key1(reg1[b]);
+        t.s2_reg_mid[b] = midcol(reg2[b]);
+        t.s2_reg_key[b] = key2(reg2[b]);
+        t.s2_reg_addr[b] = d->F[st_idx_of_canon[reg2[b]]];
+    }
+    t.eb = (int8_t)eb;
+    for (int c = 0; c < eb; ++c) t.e_log[c] = d->log_canon[c];
+    t.t1_lo = (int8_t)(s1.t_hi - r1 + 1);
+    t.t2_lo = (int8_t)(s2.t_hi - r2 + 1);
+    t.r1 = (int8_t)r1;
+    t.r2 = (int8_t)r2;
+    d->tma = t;
+    d->kernel = QFT_KERNEL_TMA2;
+    d->log2_threads = lt;
+}
+
 // Turn a PassSpec into the kernel descriptor given the current layout; updates qubit_at.
-bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, std::vector<int>& qubit_at,
-                QftPassDesc* d, std::string* err) {
+bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma,
+                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err) {
     std::memset(d, 0, sizeof(*d));
     const int f = (int)ps.F.size();
     if (f > QFT_MAX_TILE_BITS || n - f > QFT_MAX_TILEIDX_BITS) { *err = "tile too large"; return false; }
@@ -281,6 +478,7 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
             fix(d->t2_canon, std::min(4, f - s2.r));
         }
     }
+    if (d->nsteps == 2 && allow_tma) lower_tma2(d, n, hub);
     // apply the permutation to the tracking
     std::vector<int> nq(qubit_at);
     for (int a : ps.F) nq[dest[a]] = qubit_at[a];
@@ -328,7 +526,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     int wmaxseen = 0;
     for (auto& ps : specs) {
         QftPassDesc d;
-        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), qubit_at, &d, err)) return 5;
+        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u), qubit_at, &d, err)) return 5;
         wmaxseen = std::max(wmaxseen, (int)ps.window.size());
         out->passes.push_back(d);
     }
@@ -409,6 +607,145 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 --next_qubit;
             }
         }
+        if (d.kernel == QFT_KERNEL_TMA2) {
+            // replay the kernel's index maps: every (thread, register) of both steps
+            const QftTma2Desc& t = d.tma;
+            const int f = d.f, lt = f - 5, nt = 1 << lt;
+            if (d.nsteps != 2 || d.log2_threads != lt) return fail("tma2: shape");
+            const QftStep s1 = d.steps[0], s2 = d.steps[1];
+            std::vector<int> canon_at_load(n, -1);
+            for (int j = 0; j < f; ++j) canon_at_load[d.F[j]] = d.ld_canon[j];
+            {
+                // landing order = the box bits of the tensor-map dims, dimension by dimension
+                int nl = 0;
+                for (int i = 0; i < 5; ++i)
+                    for (int b = 0; b < t.tma_box[i]; ++b) {
+                        if (nl >= f || t.land_addr[nl] != t.tma_lo[i] + b) return fail("tma2: land_addr");
+                        if (t.land_addr[nl] < 0 || t.land_addr[nl] >= n || canon_at_load[t.land_addr[nl]] < 0) return fail("tma2: landing bit outside the tile");
+                        ++nl;
+                    }
+                if (nl != f) return fail("tma2: landing bits");
+            }
+            // canonical index of (tid, B) in each step, recovered from the load / store columns
+            auto canon1 = [&](int tid, int B) {
+                uint32_t off = 0;
+                for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) off ^= t.s1_tid_ld[j];
+                for (int b = 0; b < 5; ++b) if ((B >> b) & 1) off ^= t.s1_reg_ld[b];
+                const uint32_t idx = off >> 3;  // load-order index
+                uint32_t c = 0;
+                for (int j = 0; j < f; ++j) if ((idx >> j) & 1u) c |= 1u << canon_at_load[t.land_addr[j]];
+                return std::make_pair(idx, c);
+            };
+            std::vector<int> mid_canon((size_t)1 << f, -1);
+            std::vector<char> seen_ld((size_t)1 << f, 0);
+            for (int tid = 0; tid < nt; ++tid) {
+                uint32_t key = 0, offm_t = 0;
+                for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) { key ^= t.s1_tid_key[j]; offm_t ^= t.s1_tid_mid[j]; }
+                for (int B = 0; B < 32; ++B) {
+                    auto ic = canon1(tid, B);
+                    if (ic.first >= (1u << f) || seen_ld[ic.first]) return fail("tma2: step 1 reads are not a bijection");
+                    seen_ld[ic.first] = 1;
+                    const uint32_t c = ic.second;
+                    // register bits [0, r1) must be group 1's canonical bits
+                    if (((c >> s1.a) & ((1u << s1.r) - 1u)) != (uint32_t)(B & ((1 << s1.r) - 1))) return fail("tma2: step 1 register bits");
+                    uint32_t kk = key, offm = offm_t;
+                    for (int b = 0; b < 5; ++b) if ((B >> b) & 1) { kk ^= t.s1_reg_key[b]; offm ^= t.s1_reg_mid[b]; }
+                    if ((B >> s1.r) == 0 || true) {
+                        const uint32_t v = (c >> s2.a) & ((1u << s2.r) - 1u);
+                        // the kernel uses key bits from thread + batch bits only; group bits contribute 0
+                        uint32_t kb = key;
+                        for (int b = s1.r; b < 5; ++b) if ((B >> b) & 1) kb ^= t.s1_reg_key[b];
+                        if ((kb & 31u) != v) return fail("tma2: step 1 key (group 2 value)");
+                        if (((kb >> 8) & 15u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
+                        for (int b = 0; b < s1.r; ++b) if (t.s1_reg_key[b]) return fail("tma2: group bit in key");
+                    }
+                    (void)kk;
+                    if (offm & 7u) return fail("tma2: mid offset alignment");
+                    const uint32_t slot = offm >> 3;
+                    if (slot >= (1u << f) || mid_canon[slot] != -1) return fail("tma2: exchange layout is not a bijection");
+                    mid_canon[slot] = (int)c;
+                }
+                // bank check: lanes 0-15 of every warp, same register, distinct 8-byte bank pairs
+            }
+            for (int w = 0; w < nt / 16; ++w) {
+                for (int pass2 = 0; pass2 < 2; ++pass2) {
+                    int banks = 0;
+                    for (int lane = 0; lane < 16; ++lane) {
+                        const int tid = w * 16 + lane;
+                        uint32_t off = 0;
+                        for (int j = 0; j < lt; ++j)
+                            if ((tid >> j) & 1) off ^= pass2 ? t.s2_tid_mid[j] : t.s1_tid_mid[j];
+                        banks |= 1 << ((off >> 3) & 15);
+                    }
+                    if (banks != 0xFFFF) return fail("tma2: exchange layout has bank conflicts");
+                }
+                int banks = 0;
+                for (int lane = 0; lane < 16; ++lane) {
+                    const int tid = w * 16 + lane;
+                    uint32_t off = 0;
+                    for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) off ^= t.s1_tid_ld[j];
+                    banks |= 1 << ((off >> 3) & 15);
+                }
+                if (banks != 0xFFFF) return fail("tma2: landing layout read with bank conflicts");
+            }
+            std::vector<char> seen_st((size_t)1 << f, 0);
+            for (int tid = 0; tid < nt; ++tid) {
+                uint32_t key = 0, offm_t = 0;
+                uint32_t st_idx_t = 0;
+                for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) {
+                    key ^= t.s2_tid_key[j]; offm_t ^= t.s2_tid_mid[j];
+                    int found = -1;
+                    for (int jj = 0; jj < f; ++jj) if (d.F[jj] == t.s2_tid_addr[j]) found = jj;
+                    if (found < 0) return fail("tma2: store address bit outside the tile");
+                    st_idx_t |= 1u << found;
+                }
+                for (int B = 0; B < 32; ++B) {
+                    uint32_t offm = offm_t, st_idx = st_idx_t;
+                    uint32_t kb = key;
+                    for (int b = 0; b < 5; ++b) if ((B >> b) & 1) {
+                        offm ^= t.s2_reg_mid[b];
+                        int found = -1;
+                        for (int jj = 0; jj < f; ++jj) if (d.F[jj] == t.s2_reg_addr[b]) found = jj;
+                        if (found < 0) return fail("tma2: store address bit outside the tile");
+                        st_idx |= 1u << found;
+                        if (b >= s2.r) kb ^= t.s2_reg_key[b];
+                    }
+                    const uint32_t slot = offm >> 3;
+                    if (slot >= (1u << f) || mid_canon[slot] < 0) return fail("tma2: step 2 reads an empty slot");
+                    const uint32_t c = (uint32_t)mid_canon[slot];
+                    if (((c >> s2.a) & ((1u << s2.r) - 1u)) != (uint32_t)(B & ((1 << s2.r) - 1))) return fail("tma2: step 2 register bits");
+                    if ((kb & 31u) != ((c >> s1.a) & ((1u << s1.r) - 1u))) return fail("tma2: step 2 key (group 1 value)");
+                    if (((kb >> 8) & 15u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
+                    // the element with canonical index c must land on store-order index st(c)
+                    uint32_t want = 0;
+                    for (int j = 0; j < f; ++j) if ((c >> d.st_canon[j]) & 1u) want |= 1u << j;
+                    if (want != st_idx) return fail("tma2: store address disagrees with the layout adapter");
+                    if (seen_st[st_idx]) return fail("tma2: stores are not a bijection");
+                    seen_st[st_idx] = 1;
+                }
+            }
+            for (int j = 0; j < std::min<int>(t.tma_box[0], 4) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
+            if (t.eb != s2.a || t.eb > 4) return fail("tma2: eb");
+            for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
+            if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
+            // tensor-map dims partition the address bits; box bits are exactly F; dim 0 starts at bit 0
+            int a = 0, boxbits = 0;
+            std::vector<int> covered(n + 1, 0);
+            if (t.tma_lo[0] != 0) return fail("tma2: dimension 0 is not the contiguous one");
+            for (int i = 0; i < 5; ++i) {
+                if (t.tma_box[i] != 0 && t.tma_box[i] != t.tma_len[i]) return fail("tma2: box");
+                if (t.tma_box[i] > 8 || t.tma_len[i] > 30) return fail("tma2: dim too large");
+                for (int b = 0; b < t.tma_len[i]; ++b) {
+                    const int bit = t.tma_lo[i] + b;
+                    if (bit < 0 || bit >= n || covered[bit]) return fail("tma2: tensor-map dims do not partition the address bits");
+                    covered[bit] = 1;
+                    if ((t.tma_box[i] != 0) != (inF[bit] != 0)) return fail("tma2: box bits are not the tile bits");
+                }
+                boxbits += t.tma_box[i];
+                a += t.tma_len[i];
+            }
+            if (a != n || boxbits != f || t.tma_box[0] < 1) return fail("tma2: tensor map does not cover the state");
+        }
         if (d.do_scale) ++nscaled;
         // permutation
         std::vector<int> nq(qubit_at);
@@ -442,7 +779,7 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
     for (size_t i = 0; i < plan.passes.size(); ++i) {
         const QftPassDesc& d = plan.passes[i];
         if (i) o << ",";
-        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic") << "\",\"tile_bits\":" << d.f
+        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2 ? "tma2" : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic") << "\",\"tile_bits\":" << d.f
           << ",\"F\":[";
         for (int j = 0; j < d.f; ++j) o << (j ? "," : "") << (int)d.F[j];
         o << "],\"window\":[";

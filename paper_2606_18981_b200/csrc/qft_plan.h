@@ -22,6 +22,10 @@
 #define QFT_MAX_TILEIDX_BITS 34
 #define QFT_MAX_STEPS 14
 #define QFT_MAX_RADIX_BITS 5
+// QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, 2 x 16 rows of end bases, one mbarrier, 5 coords
+#define QFT_TMA2_MID_STRIDE 8   // float2 per row (R1 <= 5 used)
+#define QFT_TMA2_END_STRIDE 16  // float2 per row (R1 + R2 <= 10 used)
+#define QFT_TMA2_TABLE_BYTES ((32 * QFT_TMA2_MID_STRIDE + 2 * 16 * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)
 
 struct QftStep {
     int8_t r;     // qubits in the group
@@ -33,6 +37,26 @@ struct QftStep {
 enum QftKernelKind : int32_t {
     QFT_KERNEL_GENERIC = 0,  // shared-memory staged tile pass, any descriptor
     QFT_KERNEL_FUSED2 = 1,   // two register steps: global -> reg -> smem -> reg -> global
+    QFT_KERNEL_TMA2 = 2,     // persistent: TMA tile load -> reg -> smem -> reg -> global, packed FP32x2
+};
+
+// QFT_KERNEL_TMA2 only.  Every shared-memory byte offset is a GF(2)-linear function of the thread
+// index and the register index, given column by column; "thread bit j" is bit j of threadIdx.x,
+// "register bit b" is bit b of the index into the thread's 32 amplitudes.  Register bits [0, r) of a
+// step are its group's qubits (ascending), the rest are batch bits.
+struct QftTma2Desc {
+    uint32_t s1_tid_ld[9], s1_reg_ld[5];    // step 1 read: the TMA landing layout (tile load order)
+    uint32_t s1_tid_mid[9], s1_reg_mid[5];  // step 1 write: the swizzled exchange layout
+    uint32_t s2_tid_mid[9], s2_reg_mid[5];  // step 2 read: the same layout seen from step 2's threads
+    uint16_t s1_tid_key[9], s1_reg_key[5];  // step 1 key: bits 0-4 = value of group 2's qubits, 8-11 = e
+    uint16_t s2_tid_key[9], s2_reg_key[5];  // step 2 key: bits 0-4 = value of group 1's qubits, 8-11 = e
+    int8_t s2_tid_addr[9], s2_reg_addr[5];  // step 2 store: HBM address bit of each thread / register bit
+    int8_t eb;                              // in-tile logical qubits below the window (<= 4); e indexes them
+    int8_t e_log[4];                        // their logical ids, ascending
+    int8_t t1_lo, t2_lo;                    // lowest logical qubit of group 1 / group 2
+    int8_t r1, r2;
+    int8_t tma_lo[5], tma_len[5], tma_box[5];  // tensor-map dims: address bits [lo, lo+len), box 2^box
+    int8_t land_addr[16];                      // landing-index bit j of the shared-memory tile <-> address bit
 };
 
 // Plain data, passed to the kernels by value (__grid_constant__).
@@ -66,6 +90,7 @@ struct QftPassDesc {
     int8_t t1_addr[16], t1_canon[16], r1_addr[QFT_MAX_RADIX_BITS + 3];
     int8_t t2_addr[16], t2_canon[16], r2_addr[QFT_MAX_RADIX_BITS + 3];
     uint8_t swz_col[16];
+    QftTma2Desc tma;
 };
 
 #include <string>

@@ -1,0 +1,317 @@
+// qft_tma.cuh -- the persistent TMA-staged two-step pass kernel (QFT_KERNEL_TMA2), sm_100a.
+//
+// One CTA owns one 2^f-amplitude shared-memory buffer and walks over tiles (stride = grid size).
+// Per tile, per amplitude: HBM --TMA--> smem -> registers -> smem -> registers -> HBM.
+//   load   : one elected thread issues cp.async.bulk.tensor (UTMALDG) for the whole tile -- a 5-D box of
+//            the state seen as a tensor over its address-bit runs -- and everybody waits on an mbarrier;
+//            no thread computes a global load address, and the load of tile i+1 is issued as soon as
+//            the buffer is free, so it is in flight while tile i is still being transformed and stored;
+//   step 1 : each thread takes the 32 amplitudes of its radix-2^R1 butterflies, applies H and the
+//            controlled-R_m onto the window's R1 highest qubits with packed FP32x2
+//            arithmetic, multiplies by the phase that group 2's qubits contribute,
+//            and writes to an XOR-swizzled exchange layout;
+//   step 2 : the same for the window's R2 lower qubits, then one more phase per amplitude: the product
+//            of every controlled-R_m from a qubit *below* the window onto any of the window's qubits.
+//            For group 1 that phase was deferred: it is diagonal in bits step 2 does not touch, so it
+//            commutes with step 2 and the two multiplications merge into one;
+//   store  : straight from registers, lanes along the hub so every warp store covers whole granules,
+//            at the addresses the layout adapter dictates; for a pair pass into the
+//            partner tile after a cluster barrier (the partner's TMA load has completed by then).
+// Phase factors are never evaluated per amplitude: per CTA 32 x R1 "mid" bases, per tile 2^eb x (R1+R2)
+// "end" bases (sincos on an exact 32-bit fraction of a turn), multiplied up along the subset tree.
+#pragma once
+#include <cuda.h>
+
+#include "qft_device.cuh"
+#include "qft_packed.cuh"
+
+namespace qftk {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                            int c3, int c4) {
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], "
+        "[%2];" ::"r"(smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
+}
+
+// Plain C++ accesses (not asm): the compiler knows they touch shared memory, keeps them on the right
+// side of __syncthreads(), and is otherwise free to schedule them among the arithmetic.
+__device__ __forceinline__ float2 lds64(const unsigned char* base, uint32_t off) {
+    return *reinterpret_cast<const float2*>(base + off);
+}
+__device__ __forceinline__ void sts64(unsigned char* base, uint32_t off, float2 v) {
+    *reinterpret_cast<float2*>(base + off) = v;
+}
+
+// XOR of the columns selected by the set bits of v
+template <typename T, int N>
+__device__ __forceinline__ T xor_cols(const T (&col)[N], uint32_t v, int nbits) {
+    T r = 0;
+    for (int j = 0; j < nbits; ++j)
+        if ((v >> j) & 1u) r ^= col[j];
+    return r;
+}
+
+// offset of register B: XOR of the register-bit columns (compile-time B, run-time columns)
+template <int B>
+__device__ __forceinline__ uint32_t reg_off(const uint32_t (&c)[5]) {
+    uint32_t r = 0;
+    if constexpr (B & 1) r ^= c[0];
+    if constexpr (B & 2) r ^= c[1];
+    if constexpr (B & 4) r ^= c[2];
+    if constexpr (B & 8) r ^= c[3];
+    if constexpr (B & 16) r ^= c[4];
+    return r;
+}
+
+constexpr int kMidStride = QFT_TMA2_MID_STRIDE;
+constexpr int kEndStride = QFT_TMA2_END_STRIDE;
+
+// Multiply the 2^R amplitudes of batch BATCH by the subset products of W (optionally times p0).
+template <int R, int BATCH, bool HASP>
+__device__ __forceinline__ void apply_tree(float2 (&x)[32], const float2 (&W)[5], float2 p0) {
+    qftp::TwTree<5, BATCH << R, R - 1, 0, HASP, 5>::run(x, W, p0);
+}
+
+template <int R, int BT, int NB, bool HASP>
+struct BatchApply {
+    static __device__ __forceinline__ void run(float2 (&x)[32], const float2 (&W)[NB][5], const float2 (&p)[NB]) {
+        apply_tree<R, BT, HASP>(x, W[BT], p[BT]);
+        if constexpr (BT + 1 < NB) BatchApply<R, BT + 1, NB, HASP>::run(x, W, p);
+    }
+};
+
+template <int R1, int R2, int KC, int LT>
+__global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
+    qft_pass_tma2(float2* __restrict__ state, const __grid_constant__ CUtensorMap tmap,
+                  const __grid_constant__ QftPassDesc d) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int F = LT + 5;
+    constexpr int NT = 1 << LT;
+    float2* midW = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F));
+    float2* endW = midW + 32 * kMidStride;
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(endW + 2 * 16 * kEndStride);  // two end tables (by parity)
+    int* nextc = reinterpret_cast<int*>(mbar + 1);                              // next tile's TMA coordinates
+    const uint32_t tid = threadIdx.x;
+    const QftTma2Desc& t = d.tma;
+
+    // ---- per-thread constants ----
+    uint32_t off1_ld = xor_cols(t.s1_tid_ld, tid, LT);
+    uint32_t off1_mid = xor_cols(t.s1_tid_mid, tid, LT);
+    uint32_t off2_mid = xor_cols(t.s2_tid_mid, tid, LT);
+    const uint32_t key1 = xor_cols(t.s1_tid_key, tid, LT);
+    const uint32_t key2 = xor_cols(t.s2_tid_key, tid, LT);
+    uint64_t st_thread = 0;
+    for (int j = 0; j < LT; ++j)
+        if ((tid >> j) & 1u) st_thread |= 1ull << t.s2_tid_addr[j];
+    uint32_t c1ld[5], c1mid[5], c2mid[5];
+    uint64_t c2st[5];
+#pragma unroll
+    for (int b = 0; b < 5; ++b) {
+        c1ld[b] = t.s1_reg_ld[b];
+        c1mid[b] = t.s1_reg_mid[b];
+        c2mid[b] = t.s2_reg_mid[b];
+        c2st[b] = 1ull << t.s2_reg_addr[b];
+    }
+    const int k = d.k;
+    const int win_lo = d.win_lo;
+    const uint64_t lbmask = (win_lo > 0) ? ((1ull << win_lo) - 1ull) : 0ull;
+
+    if (tid == 0) {
+        mbar_init(mbar, 1);
+        fence_proxy_async();
+    }
+    // mid bases: midW[v][i] = product of the controlled-R_m from group 2's qubits (value v) onto
+    // group 1's i-th qubit
+    for (uint32_t i = tid; i < 32u * R1; i += NT) {
+        const uint32_t v = i / R1, q = i % R1;
+        midW[v * kMidStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32((uint64_t)v << t.t2_lo, t.t1_lo + (int)q, k));
+    }
+    __syncthreads();
+
+    // ---- tile walk ----
+    const uint32_t csz = d.npair ? 2u : 1u;
+    const uint32_t rho = d.npair ? (blockIdx.x & 1u) : 0u;
+    const uint32_t nunits = (1u << d.ntile) / csz;
+    const uint32_t ustride = gridDim.x / csz;
+    const bool has_end = win_lo > 0;
+
+    // tile index -> TMA coordinates (HBM address bits of the tile, cut into the tensor map's dims)
+    auto coords_of = [&](uint32_t un, int (&c)[5]) {
+        uint32_t ml, ms;
+        decode_tile(un * csz + rho, d.npair, &ml, &ms);
+        uint64_t base = 0;
+        for (int i = 0; i < d.ntile; ++i)
+            if ((ml >> i) & 1u) base |= 1ull << d.tile_addr[i];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) c[j] = (int)((base >> t.tma_lo[j]) & ((1ull << t.tma_len[j]) - 1ull));
+    };
+
+    uint32_t unit = blockIdx.x / csz;
+    if (unit < nunits && tid == 0) {
+        int c[5];
+        coords_of(unit, c);
+        mbar_expect_tx(mbar, 8u << F);
+        tma_load_5d(smem_raw, &tmap, mbar, c[0], c[1], c[2], c[3], c[4]);
+    }
+    uint32_t parity = 0;
+    for (; unit < nunits; unit += ustride) {
+        // ---- bookkeeping while the tile's load is in flight (few registers live here) ----
+        uint64_t base_st = 0;
+        float2* endWp = endW + parity * (16 * kEndStride);
+        {
+            uint32_t ml, ms;
+            decode_tile(unit * csz + rho, d.npair, &ml, &ms);
+            uint64_t Ltile = 0;
+            for (int i = 0; i < d.ntile; ++i) {
+                if ((ml >> i) & 1u) Ltile |= 1ull << d.log_tile[i];
+                if ((ms >> i) & 1u) base_st |= 1ull << d.tile_addr[i];
+            }
+            if (has_end) {
+                // end bases of this tile: endW[e][q] = product of the controlled-R_m from every qubit
+                // below the window (tile-index bits + in-tile bits e) onto the window's q-th qubit
+                const uint32_t nq = R1 + R2;
+                const uint32_t cnt = nq << t.eb;
+                for (uint32_t i = tid; i < cnt; i += NT) {
+                    const uint32_t e = i / nq, q = i % nq;
+                    uint64_t L = Ltile;
+                    for (int b = 0; b < t.eb; ++b)
+                        if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
+                    L &= lbmask;
+                    endWp[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, win_lo + (int)q, k));
+                }
+            }
+            if (tid == 0 && unit + ustride < nunits) {
+                int c[5];
+                coords_of(unit + ustride, c);
+#pragma unroll
+                for (int j = 0; j < 5; ++j) nextc[j] = c[j];
+            }
+        }
+        float2 x[32];
+        // keep the 96 per-register shared-memory offsets out of loop-invariant hoisting (they would
+        // spill): one XOR next to each access is cheaper than a local-memory reload
+        asm volatile("" : "+r"(off1_ld), "+r"(off1_mid), "+r"(off2_mid));
+        mbar_wait(mbar, parity);
+        if (d.npair) cluster_arrive();  // this CTA's tile is on chip: the partner may overwrite it in HBM
+
+        // ------------------------------ step 1 ------------------------------
+#define QFT_LD1(B) x[B] = lds64(smem_raw, off1_ld ^ reg_off<B>(c1ld));
+#define QFT_ALL32(M)                                                                                          \
+    M(0) M(1) M(2) M(3) M(4) M(5) M(6) M(7) M(8) M(9) M(10) M(11) M(12) M(13) M(14) M(15) M(16) M(17) M(18)  \
+        M(19) M(20) M(21) M(22) M(23) M(24) M(25) M(26) M(27) M(28) M(29) M(30) M(31)
+        QFT_ALL32(QFT_LD1)
+#undef QFT_LD1
+        __syncthreads();  // every amplitude of the tile is in a register: the buffer becomes the exchange
+        if (d.conj) {
+#pragma unroll
+            for (int B = 0; B < 32; ++B) x[B].y = -x[B].y;
+        }
+        qftp::dif_group<5, R1, KC>(x);
+        {
+            constexpr int NB1 = 1 << (5 - R1);
+            float2 W1[NB1][5];
+            float2 one[NB1];
+#pragma unroll
+            for (int bt = 0; bt < NB1; ++bt) {
+                uint32_t kk = key1;
+#pragma unroll
+                for (int i = 0; i < 5 - R1; ++i)
+                    if (bt & (1 << i)) kk ^= t.s1_reg_key[R1 + i];
+                const float2* row = midW + (kk & 31u) * kMidStride;
+#pragma unroll
+                for (int i = 0; i < R1; ++i) W1[bt][i] = row[i];
+                one[bt] = make_float2(1.f, 0.f);
+            }
+            BatchApply<R1, 0, NB1, false>::run(x, W1, one);
+        }
+#define QFT_ST1(B) sts64(smem_raw, off1_mid ^ reg_off<B>(c1mid), x[B]);
+        QFT_ALL32(QFT_ST1)
+#undef QFT_ST1
+        __syncthreads();
+
+        // ------------------------------ step 2 ------------------------------
+#define QFT_LD2(B) x[B] = lds64(smem_raw, off2_mid ^ reg_off<B>(c2mid));
+        QFT_ALL32(QFT_LD2)
+#undef QFT_LD2
+        fence_proxy_async();
+        __syncthreads();  // the buffer is free again
+        if (tid == 0 && unit + ustride < nunits) {
+            // prefetch the next tile while this one is transformed and stored
+            mbar_expect_tx(mbar, 8u << F);
+            tma_load_5d(smem_raw, &tmap, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
+        }
+
+        qftp::dif_group<5, R2, KC>(x);
+        if (has_end) {
+            constexpr int NB2 = 1 << (5 - R2);
+            float2 W2[NB2][5];
+            float2 cfac[NB2];
+#pragma unroll
+            for (int bt = 0; bt < NB2; ++bt) {
+                uint32_t kk = key2;
+#pragma unroll
+                for (int i = 0; i < 5 - R2; ++i)
+                    if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
+                const float2* row = endWp + ((kk >> 8) & 15u) * kEndStride;
+#pragma unroll
+                for (int i = 0; i < R2; ++i) W2[bt][i] = row[i];
+                float2 c = make_float2(d.scale, 0.f);
+#pragma unroll
+                for (int i = 0; i < R1; ++i) {
+                    const float2 w = row[R2 + i];
+                    const float2 cw = qftp::cmul(c, w);
+                    if ((kk >> i) & 1u) c = cw;
+                }
+                cfac[bt] = c;
+            }
+            BatchApply<R2, 0, NB2, true>::run(x, W2, cfac);
+        } else if (d.do_scale) {
+#pragma unroll
+            for (int B = 0; B < 32; ++B) x[B] = qftp::cscale(x[B], d.scale);
+        }
+        if (d.conj) {
+#pragma unroll
+            for (int B = 0; B < 32; ++B) x[B].y = -x[B].y;
+        }
+        if (d.npair) cluster_wait();  // the partner holds its tile on chip: its addresses may be overwritten
+        float2* __restrict__ dst = state + (base_st | st_thread);
+#pragma unroll
+        for (int B = 0; B < 32; ++B) {
+            uint64_t o = 0;
+#pragma unroll
+            for (int b = 0; b < 5; ++b)
+                if (B & (1 << b)) o += c2st[b];
+            dst[o] = x[B];
+        }
+        parity ^= 1u;
+    }
+#undef QFT_ALL32
+}
+
+}  // namespace qftk

@@ -1,0 +1,25 @@
+// qft_tma_inst.cuh -- kernel-pointer tables of qft_pass_tma2 per (R1, R2, KC) for one thread count.
+#pragma once
+#include "qft_tma.cuh"
+
+typedef void (*tma2_kernel_t)(float2*, const CUtensorMap, const QftPassDesc);
+
+template <int R1, int R2, int LT>
+static tma2_kernel_t qft_pick_tma2_kc(int kc) {
+    switch (kc) {
+        case 0: return qftk::qft_pass_tma2<R1, R2, 0, LT>;
+        case 1: return qftk::qft_pass_tma2<R1, R2, 1, LT>;
+        case 2: return qftk::qft_pass_tma2<R1, R2, 2, LT>;
+        case 3: return qftk::qft_pass_tma2<R1, R2, 3, LT>;
+        default: return qftk::qft_pass_tma2<R1, R2, 4, LT>;
+    }
+}
+
+#define QFT_TMA2_DEFINE_PICK(LT)                                          \
+    tma2_kernel_t qft_pick_tma2_lt##LT(int r1, int r2, int kc) {          \
+        if (r1 == 5 && r2 == 5) return qft_pick_tma2_kc<5, 5, LT>(kc);    \
+        if (r1 == 5 && r2 == 4) return qft_pick_tma2_kc<5, 4, LT>(kc);    \
+        if (r1 == 4 && r2 == 4) return qft_pick_tma2_kc<4, 4, LT>(kc);    \
+        if (r1 == 4 && r2 == 3) return qft_pick_tma2_kc<4, 3, LT>(kc);    \
+        return nullptr;                                                   \
+    }

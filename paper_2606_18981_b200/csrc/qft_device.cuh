@@ -192,6 +192,10 @@ __device__ __forceinline__ float2 ld_stream(const float2* p) {
     return v;
 }
 
+// Relaxed arrive for the TMA kernels: the arriving CTA only announces "my tile is on chip" (it has
+// observed its own mbarrier), it publishes no writes, so the release fence (a MEMBAR that waits for
+// the previous tile's stores to drain) is not needed.
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 

@@ -13,6 +13,7 @@
 //      cluster barrier (both CTAs of the pair have finished loading by then, so in place is safe).
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include "qft_device.cuh"
 #include "qft_fused.cuh"
@@ -225,6 +226,11 @@ int g_qft_tma_l2promo = 1;  // CUtensorMapL2promotion: 0 none, 1 64 B, 2 128 B, 
 static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t stream) {
     tma2_kernel_t kern = pick_tma2(d);
     encode_tiled_t enc = get_encode_tiled();
+    static const int promo_env = []() {
+        const char* e = getenv("QFT_TMA_L2PROMO");
+        return e ? atoi(e) : -1;
+    }();
+    if (promo_env >= 0 && promo_env <= 3) g_qft_tma_l2promo = promo_env;
     if (!kern || !enc) return cudaErrorNotSupported;
     CUtensorMap map;
     cuuint64_t gdim[5], gstr[4];

@@ -213,7 +213,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
     if (!((r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3))) return;
     if (s1.a != s2.a + r2) return;  // the window is one run of canonical bits
     const int eb = s2.a;            // canonical bits below the window
-    if (eb > 4) return;
+    if (eb > 5) return;
     if (n - f < 1) return;
     (void)hub;
     QftTma2Desc t;
@@ -235,7 +235,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
     // the four lowest landing-index bits (conflict-free reads by lanes that run along the low bits).
     struct Dim { int lo, len, box, cls; };
     std::vector<Dim> dims;
-    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return in1(c) ? 2 : (in2(c) ? 1 : 0); };
+    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return in1(c) ? 2 : 0; };
     int a = 0;
     while (a < n) {
         int b = a + 1;
@@ -656,7 +656,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                         uint32_t kb = key;
                         for (int b = s1.r; b < 5; ++b) if ((B >> b) & 1) kb ^= t.s1_reg_key[b];
                         if ((kb & 31u) != v) return fail("tma2: step 1 key (group 2 value)");
-                        if (((kb >> 8) & 15u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
+                        if (((kb >> 8) & 31u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
                         for (int b = 0; b < s1.r; ++b) if (t.s1_reg_key[b]) return fail("tma2: group bit in key");
                     }
                     (void)kk;
@@ -715,7 +715,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     const uint32_t c = (uint32_t)mid_canon[slot];
                     if (((c >> s2.a) & ((1u << s2.r) - 1u)) != (uint32_t)(B & ((1 << s2.r) - 1))) return fail("tma2: step 2 register bits");
                     if ((kb & 31u) != ((c >> s1.a) & ((1u << s1.r) - 1u))) return fail("tma2: step 2 key (group 1 value)");
-                    if (((kb >> 8) & 15u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
+                    if (((kb >> 8) & 31u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
                     // the element with canonical index c must land on store-order index st(c)
                     uint32_t want = 0;
                     for (int j = 0; j < f; ++j) if ((c >> d.st_canon[j]) & 1u) want |= 1u << j;
@@ -725,7 +725,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 }
             }
             for (int j = 0; j < std::min<int>(t.tma_box[0], 4) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
-            if (t.eb != s2.a || t.eb > 4) return fail("tma2: eb");
+            if (t.eb != s2.a || t.eb > 5) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
             // tensor-map dims partition the address bits; box bits are exactly F; dim 0 starts at bit 0

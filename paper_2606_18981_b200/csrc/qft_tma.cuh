@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     constexpr int NT = 1 << LT;
     float2* midW = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F));
     float2* endW = midW + 32 * kMidStride;
-    uint64_t* mbar = reinterpret_cast<uint64_t*>(endW + 2 * 16 * kEndStride);  // two end tables (by parity)
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(endW + 2 * 32 * kEndStride);  // two end tables (by parity)
     int* nextc = reinterpret_cast<int*>(mbar + 1);                              // next tile's TMA coordinates
     const uint32_t tid = threadIdx.x;
     const QftTma2Desc& t = d.tma;
@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     for (; unit < nunits; unit += ustride) {
         // ---- bookkeeping while the tile's load is in flight (few registers live here) ----
         uint64_t base_st = 0;
-        float2* endWp = endW + parity * (16 * kEndStride);
+        float2* endWp = endW + parity * (32 * kEndStride);
         {
             uint32_t ml, ms;
             decode_tile(unit * csz + rho, d.npair, &ml, &ms);
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         // spill): one XOR next to each access is cheaper than a local-memory reload
         asm volatile("" : "+r"(off1_ld), "+r"(off1_mid), "+r"(off2_mid));
         mbar_wait(mbar, parity);
-        if (d.npair) cluster_arrive();  // this CTA's tile is on chip: the partner may overwrite it in HBM
+        if (d.npair) cluster_arrive_relaxed();  // this CTA's tile is on chip: the partner may overwrite it in HBM
 
         // ------------------------------ step 1 ------------------------------
 #define QFT_LD1(B) x[B] = lds64(smem_raw, off1_ld ^ reg_off<B>(c1ld));
@@ -278,7 +278,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
 #pragma unroll
                 for (int i = 0; i < 5 - R2; ++i)
                     if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
-                const float2* row = endWp + ((kk >> 8) & 15u) * kEndStride;
+                const float2* row = endWp + ((kk >> 8) & 31u) * kEndStride;
 #pragma unroll
                 for (int i = 0; i < R2; ++i) W2[bt][i] = row[i];
                 float2 c = make_float2(d.scale, 0.f);

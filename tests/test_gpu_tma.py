@@ -1,0 +1,70 @@
+"""GPU parity of the TMA-staged pass kernel (tma2) against the CPU oracle, element by element.
+
+The sizes (n = 20 ... 24) are the smallest at which the planner emits tma2 passes, chosen so that the
+tile / hub knobs of qft_plan_create_tuned put it in every position (first pass with the hub swap, mid
+pass with the 2-CTA-cluster pair store, last pass with the scale), with every register-group shape
+(4+3, 4+4, 5+4, 5+5 only at n >= 28: tests/test_gpu_large.py) and every in-group AQFT truncation
+(k = 0 ... 3 and k >= 4 are separate kernel instantiations).  Tolerance: north_star's 2e-5 (n <= 20),
+1e-4 above.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import qft_inputs as qi
+
+pytestmark = pytest.mark.gpu
+
+CFGS = [(20, 12, 3), (20, 13, 3), (21, 12, 4), (22, 13, 3), (22, 13, 4), (22, 12, 4), (23, 14, 4), (24, 13, 3),
+        (24, 14, 4), (24, 12, 3), (24, 12, 4)]
+VARIANTS = [(None, -1, 0), (3, -1, 0), (1, 1, 1), (None, 1, 2), (0, -1, 0), (2, -1, 0), (9, -1, 0)]
+
+
+@pytest.mark.parametrize("n,tile_bits,hub_bits", CFGS)
+def test_tma2_against_oracle(n, tile_bits, hub_bits):
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    x = qi.gaussian(n, n)
+    saw_tma2 = False
+    for k, sign, norm in VARIANTS:
+        kk = n if k is None else k
+        plan = qft.Plan(n, kk, 13, sign, norm, tile_bits, hub_bits, 0)
+        plan.self_check()
+        kinds = [p["kernel"] for p in plan.describe()["passes"]]
+        saw_tma2 |= "tma2" in kinds
+        t = torch.from_numpy(x).cuda()
+        plan.execute(t)
+        torch.cuda.synchronize()
+        got = t.cpu().numpy().astype(np.complex128)
+        plan.close()
+        ref = oracle.qft(x, kk, sign, norm)
+        err = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+        assert err <= (2e-5 if n <= 20 else 1e-4), (n, tile_bits, hub_bits, kk, sign, norm, kinds, err)
+    assert saw_tma2, "this configuration was chosen to exercise the tma2 kernel"
+
+
+def test_tma2_matches_generic_kernel_bitwise_layout():
+    """Same plan with and without the fused kernels (flags = QFT_FLAG_GENERIC_ONLY): the generic
+    shared-memory kernel is the slow reference implementation of the same pass list, so the two
+    results must agree to rounding; a tone input must land in one bin."""
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    n = 25
+    x = qi.tone(n, 12345)
+    outs = []
+    for flags in (0, qft.QFT_FLAG_GENERIC_ONLY):
+        plan = qft.Plan(n, n, 13, -1, 0, 13, 4, flags)
+        t = torch.from_numpy(x).cuda()
+        plan.execute(t)
+        torch.cuda.synchronize()
+        outs.append(t)
+        plan.close()
+    d = float(torch.linalg.vector_norm(outs[0] - outs[1]).item())
+    assert d <= 1e-5
+    peak = int(torch.argmax(outs[0].abs()).item())
+    assert peak == 12345
+    assert abs(abs(outs[0][peak].item()) - 1.0) <= 1e-4

@@ -91,6 +91,8 @@ qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, i
  */
 #define QFT_FLAG_GENERIC_ONLY 1u  /* use only the generic shared-memory tile kernel */
 #define QFT_FLAG_UNFOLDED 2u      /* natural-order passes + one stand-alone bit-reversal pass */
+#define QFT_FLAG_NO_TMA 4u        /* do not use the TMA-staged pass kernels */
+#define QFT_FLAG_PINGPONG 8u      /* tile_bits = 14 only: two-group ping-pong variant of the TMA kernel (experimental, slower) */
 qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                                    qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
 

@@ -184,9 +184,11 @@ typedef void (*tma2_kernel_t)(float2*, const CUtensorMap, const QftPassDesc);
 tma2_kernel_t qft_pick_tma2_lt7(int r1, int r2, int kc);  // qft_tma_lt7.cu
 tma2_kernel_t qft_pick_tma2_lt8(int r1, int r2, int kc);  // qft_tma_lt8.cu
 tma2_kernel_t qft_pick_tma2_lt9(int r1, int r2, int kc);  // qft_tma_lt9.cu
+tma2_kernel_t qft_pick_tma2pp(int r1, int r2, int kc);    // qft_tma_pp.cu
 
 static tma2_kernel_t pick_tma2(const QftPassDesc& d) {
     const int kc = d.k < 4 ? d.k : 4;
+    if (d.kernel == QFT_KERNEL_TMA2PP) return qft_pick_tma2pp(d.tma.r1, d.tma.r2, kc);
     switch (d.log2_threads) {
         case 7: return qft_pick_tma2_lt7(d.tma.r1, d.tma.r2, kc);
         case 8: return qft_pick_tma2_lt8(d.tma.r1, d.tma.r2, kc);
@@ -242,10 +244,12 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
         if (i > 0) gstr[i - 1] = 8ull << d.tma.tma_lo[i];
     }
     CUresult r = enc(&map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 5, state, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     CU_TENSOR_MAP_SWIZZLE_NONE, (CUtensorMapL2promotion)g_qft_tma_l2promo,
+                     d.kernel == QFT_KERNEL_TMA2PP ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                     (CUtensorMapL2promotion)g_qft_tma_l2promo,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES;
+    const bool pp = d.kernel == QFT_KERNEL_TMA2PP;
+    const size_t smem = pp ? (size_t)QFT_TMA2PP_SMEM_BYTES : ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES;
     cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int per_sm = d.f == 13 ? 2 : (d.f == 12 ? 4 : 1);
@@ -274,7 +278,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
 }
 
 cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream) {
-    if (d.kernel == QFT_KERNEL_TMA2) return launch_tma2(d, state, stream);
+    if (d.kernel == QFT_KERNEL_TMA2 || d.kernel == QFT_KERNEL_TMA2PP) return launch_tma2(d, state, stream);
     pass_kernel_t kern = pick_kernel(d);
     const size_t smem = (size_t)8 << d.f;
     if (smem > 48 * 1024) {

@@ -205,8 +205,9 @@ bool solve_swizzle(const int (&L1)[4], const int (&L2)[4], int f, uint8_t (&lowm
 }
 
 // Fills d->tma and sets d->kernel = QFT_KERNEL_TMA2 when the pass fits the kernel's shape.
-void lower_tma2(QftPassDesc* d, int n, int hub) {
+void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     const int f = d->f;
+    if (pp && f != 14) return;
     const QftStep s1 = d->steps[0], s2 = d->steps[1];
     const int r1 = s1.r, r2 = s2.r;
     if (f < 12 || f > 14) return;
@@ -241,7 +242,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
         int b = a + 1;
         if (inF[a]) {
             // dimension 0 may mix classes (it is the hub); the others may not
-            while (b < n && inF[b] && b - a < 8 && (cls_of(b) == cls_of(a))) ++b;
+            while (b < n && inF[b] && b - a < ((pp && a == 0) ? 4 : 8) && (cls_of(b) == cls_of(a))) ++b;
             dims.push_back({a, b - a, b - a, cls_of(a)});
         } else {
             while (b < n && !inF[b] && b - a < 30) ++b;
@@ -272,15 +273,31 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
     // step 1: register bits = group 1 (+ batch bits: the highest landing bits outside the group);
     // thread bits = the remaining landing bits, ascending, so lanes read consecutive shared memory
     std::vector<int> reg1, thr1, reg2, thr2;
+    int gcan = -1;  // ping-pong: the canonical bit that splits the tile between the two thread groups
+    if (pp) {
+        if (dims[0].box != 4) return;
+        gcan = canon_at_load[t.land_addr[3]];
+        if (in1(gcan) || in2(gcan)) return;
+    }
     for (int b = 0; b < r1; ++b) reg1.push_back(s1.a + b);
     {
         std::vector<int> rest;
         for (int j = 0; j < f; ++j) {
             const int c = canon_at_load[t.land_addr[j]];
-            if (!in1(c)) rest.push_back(c);
+            if (!in1(c) && c != gcan) rest.push_back(c);
         }
         while ((int)reg1.size() < 5) { reg1.push_back(rest.back()); rest.pop_back(); }
         thr1 = rest;
+        if (pp) {
+            // lanes 0-2 = hub bits 0-2, lane 3 = landing row bit 2 (landing index bit 6): with the 128B
+            // swizzle a half-warp then covers all 32 banks; the group bit is the top thread bit
+            const int c6 = canon_at_load[t.land_addr[6]];
+            auto it = std::find(thr1.begin(), thr1.end(), c6);
+            if (it == thr1.end() || (it - thr1.begin()) < 3) return;
+            thr1.erase(it);
+            thr1.insert(thr1.begin() + 3, c6);
+            thr1.push_back(gcan);
+        }
     }
     // step 2: register bits = group 2 (+ batch bits); thread bits = the remaining store-order bits,
     // ascending, so lanes run along the hub and every warp store covers whole granules
@@ -288,23 +305,41 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
     {
         std::vector<int> rest;
         for (int j = 0; j < f; ++j)
-            if (!in2(d->st_canon[j])) rest.push_back(d->st_canon[j]);
+            if (!in2(d->st_canon[j]) && d->st_canon[j] != gcan) rest.push_back(d->st_canon[j]);
         while ((int)reg2.size() < 5) { reg2.push_back(rest.back()); rest.pop_back(); }
         thr2 = rest;
+        if (pp) thr2.push_back(gcan);
     }
     if ((int)thr1.size() != lt || (int)thr2.size() != lt) return;
-    for (int j = 0; j < 4; ++j)
-        if (land_idx_of_canon[thr1[j]] != j) return;
-    const int hubrun = dims[0].box;
-    for (int j = 0; j < std::min(hubrun, 4); ++j)
-        if (st_idx_of_canon[thr2[j]] != j) return;
+    if (pp) {
+        for (int j = 0; j < 3; ++j)
+            if (land_idx_of_canon[thr1[j]] != j || st_idx_of_canon[thr2[j]] != j) return;
+        for (int c : reg1) if (c == gcan) return;
+        for (int c : reg2) if (c == gcan) return;
+    } else {
+        for (int j = 0; j < 4; ++j)
+            if (land_idx_of_canon[thr1[j]] != j) return;
+        const int hubrun = dims[0].box;
+        for (int j = 0; j < std::min(hubrun, 4); ++j)
+            if (st_idx_of_canon[thr2[j]] != j) return;
+    }
+    // exchange layout: canonical index (ping-pong: with the group bit squeezed out) XOR-swizzled
+    auto xpos = [&](int c) { return (gcan >= 0 && c > gcan) ? c - 1 : c; };
     int L1[4], L2[4];
-    for (int j = 0; j < 4; ++j) { L1[j] = thr1[j]; L2[j] = thr2[j]; }
+    for (int j = 0; j < 4; ++j) { L1[j] = xpos(thr1[j]); L2[j] = xpos(thr2[j]); }
     uint8_t lowmask[16];
     if (!solve_swizzle(L1, L2, f, lowmask)) return;
     auto midcol = [&](int c) -> uint32_t {
-        const uint32_t slot = (c < 4) ? (1u << c) : ((1u << c) ^ lowmask[c]);
+        if (c == gcan) return 0u;
+        const int p = xpos(c);
+        const uint32_t slot = (p < 4) ? (1u << p) : ((1u << p) ^ lowmask[p]);
         return slot << 3;
+    };
+    auto landcol = [&](int c) -> uint32_t {
+        const int j = land_idx_of_canon[c];
+        uint32_t col = 8u << j;
+        if (pp && j >= 4 && j <= 6) col ^= 16u << (j - 4);  // TMA 128B swizzle: byte bits 4-6 ^= bits 7-9
+        return col;
     };
     auto key1 = [&](int c) -> uint16_t {
         if (in2(c)) return (uint16_t)(1u << (c - s2.a));
@@ -317,7 +352,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
         return 0;
     };
     for (int j = 0; j < lt; ++j) {
-        t.s1_tid_ld[j] = 8u << land_idx_of_canon[thr1[j]];
+        t.s1_tid_ld[j] = landcol(thr1[j]);
         t.s1_tid_mid[j] = midcol(thr1[j]);
         t.s1_tid_key[j] = key1(thr1[j]);
         t.s2_tid_mid[j] = midcol(thr2[j]);
@@ -325,7 +360,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
         t.s2_tid_addr[j] = d->F[st_idx_of_canon[thr2[j]]];
     }
     for (int b = 0; b < 5; ++b) {
-        t.s1_reg_ld[b] = 8u << land_idx_of_canon[reg1[b]];
+        t.s1_reg_ld[b] = landcol(reg1[b]);
         t.s1_reg_mid[b] = midcol(reg1[b]);
         t.s1_reg_key[b] = key1(reg1[b]);
         t.s2_reg_mid[b] = midcol(reg2[b]);
@@ -338,13 +373,14 @@ void lower_tma2(QftPassDesc* d, int n, int hub) {
     t.t2_lo = (int8_t)(s2.t_hi - r2 + 1);
     t.r1 = (int8_t)r1;
     t.r2 = (int8_t)r2;
+    t.pp = pp ? 1 : 0;
     d->tma = t;
-    d->kernel = QFT_KERNEL_TMA2;
+    d->kernel = pp ? QFT_KERNEL_TMA2PP : QFT_KERNEL_TMA2;
     d->log2_threads = lt;
 }
 
 // Turn a PassSpec into the kernel descriptor given the current layout; updates qubit_at.
-bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma,
+bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma, bool allow_pp,
                 std::vector<int>& qubit_at, QftPassDesc* d, std::string* err) {
     std::memset(d, 0, sizeof(*d));
     const int f = (int)ps.F.size();
@@ -478,7 +514,8 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
             fix(d->t2_canon, std::min(4, f - s2.r));
         }
     }
-    if (d->nsteps == 2 && allow_tma) lower_tma2(d, n, hub);
+    if (d->nsteps == 2 && allow_tma && allow_pp) lower_tma2(d, n, hub, true);
+    if (d->nsteps == 2 && allow_tma && d->kernel != QFT_KERNEL_TMA2PP) lower_tma2(d, n, hub, false);
     // apply the permutation to the tracking
     std::vector<int> nq(qubit_at);
     for (int a : ps.F) nq[dest[a]] = qubit_at[a];
@@ -526,7 +563,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     int wmaxseen = 0;
     for (auto& ps : specs) {
         QftPassDesc d;
-        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u), qubit_at, &d, err)) return 5;
+        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u), (prm.flags & 8u) != 0, qubit_at, &d, err)) return 5;
         wmaxseen = std::max(wmaxseen, (int)ps.window.size());
         out->passes.push_back(d);
     }
@@ -607,7 +644,9 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 --next_qubit;
             }
         }
-        if (d.kernel == QFT_KERNEL_TMA2) {
+        if (d.kernel == QFT_KERNEL_TMA2 || d.kernel == QFT_KERNEL_TMA2PP) {
+            const bool pp = d.kernel == QFT_KERNEL_TMA2PP;
+            if (pp != (d.tma.pp != 0) || (pp && d.f != 14)) return fail("tma2pp: flag");
             // replay the kernel's index maps: every (thread, register) of both steps
             const QftTma2Desc& t = d.tma;
             const int f = d.f, lt = f - 5, nt = 1 << lt;
@@ -631,12 +670,15 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 uint32_t off = 0;
                 for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) off ^= t.s1_tid_ld[j];
                 for (int b = 0; b < 5; ++b) if ((B >> b) & 1) off ^= t.s1_reg_ld[b];
-                const uint32_t idx = off >> 3;  // load-order index
+                if (pp) off ^= ((off >> 7) & 7u) << 4;  // undo TMA's 128B swizzle
+                const uint32_t idx = off >> 3;  // landing index
                 uint32_t c = 0;
                 for (int j = 0; j < f; ++j) if ((idx >> j) & 1u) c |= 1u << canon_at_load[t.land_addr[j]];
                 return std::make_pair(idx, c);
             };
-            std::vector<int> mid_canon((size_t)1 << f, -1);
+            const int ngrp = pp ? 2 : 1;
+            const uint32_t xslots = pp ? (1u << (f - 1)) : (1u << f);
+            std::vector<int> mid_canon((size_t)ngrp << f, -1);
             std::vector<char> seen_ld((size_t)1 << f, 0);
             for (int tid = 0; tid < nt; ++tid) {
                 uint32_t key = 0, offm_t = 0;
@@ -662,8 +704,9 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     (void)kk;
                     if (offm & 7u) return fail("tma2: mid offset alignment");
                     const uint32_t slot = offm >> 3;
-                    if (slot >= (1u << f) || mid_canon[slot] != -1) return fail("tma2: exchange layout is not a bijection");
-                    mid_canon[slot] = (int)c;
+                    const size_t gs = ((size_t)(pp ? (tid >> 8) : 0) << f) + slot;
+                    if (slot >= xslots || mid_canon[gs] != -1) return fail("tma2: exchange layout is not a bijection");
+                    mid_canon[gs] = (int)c;
                 }
                 // bank check: lanes 0-15 of every warp, same register, distinct 8-byte bank pairs
             }
@@ -711,8 +754,9 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                         if (b >= s2.r) kb ^= t.s2_reg_key[b];
                     }
                     const uint32_t slot = offm >> 3;
-                    if (slot >= (1u << f) || mid_canon[slot] < 0) return fail("tma2: step 2 reads an empty slot");
-                    const uint32_t c = (uint32_t)mid_canon[slot];
+                    const size_t gs = ((size_t)(pp ? (tid >> 8) : 0) << f) + slot;
+                    if (slot >= xslots || mid_canon[gs] < 0) return fail("tma2: step 2 reads an empty slot");
+                    const uint32_t c = (uint32_t)mid_canon[gs];
                     if (((c >> s2.a) & ((1u << s2.r) - 1u)) != (uint32_t)(B & ((1 << s2.r) - 1))) return fail("tma2: step 2 register bits");
                     if ((kb & 31u) != ((c >> s1.a) & ((1u << s1.r) - 1u))) return fail("tma2: step 2 key (group 1 value)");
                     if (((kb >> 8) & 31u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
@@ -724,7 +768,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     seen_st[st_idx] = 1;
                 }
             }
-            for (int j = 0; j < std::min<int>(t.tma_box[0], 4) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
+            for (int j = 0; j < (pp ? 3 : std::min<int>(t.tma_box[0], 4)) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
             if (t.eb != s2.a || t.eb > 5) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
@@ -779,7 +823,7 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
     for (size_t i = 0; i < plan.passes.size(); ++i) {
         const QftPassDesc& d = plan.passes[i];
         if (i) o << ",";
-        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2 ? "tma2" : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic") << "\",\"tile_bits\":" << d.f
+        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2PP ? "tma2pp" : d.kernel == QFT_KERNEL_TMA2 ? "tma2" : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic") << "\",\"tile_bits\":" << d.f
           << ",\"F\":[";
         for (int j = 0; j < d.f; ++j) o << (j ? "," : "") << (int)d.F[j];
         o << "],\"window\":[";

@@ -25,6 +25,8 @@
 // QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, 2 x 32 rows of end bases, one mbarrier, 5 coords
 #define QFT_TMA2_MID_STRIDE 8   // float2 per row (R1 <= 5 used)
 #define QFT_TMA2_END_STRIDE 16  // float2 per row (R1 + R2 <= 10 used)
+// QFT_KERNEL_TMA2PP: 1 KB alignment slack + landing (2^14) + exchange (2^13) + mid + 4 end tables + mbarrier etc.
+#define QFT_TMA2PP_SMEM_BYTES (1024 + (8 << 14) + (8 << 13) + (32 * QFT_TMA2_MID_STRIDE + 4 * 32 * QFT_TMA2_END_STRIDE) * 8 + 8 + 48 + 8)
 #define QFT_TMA2_TABLE_BYTES ((32 * QFT_TMA2_MID_STRIDE + 2 * 32 * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)
 
 struct QftStep {
@@ -38,6 +40,7 @@ enum QftKernelKind : int32_t {
     QFT_KERNEL_GENERIC = 0,  // shared-memory staged tile pass, any descriptor
     QFT_KERNEL_FUSED2 = 1,   // two register steps: global -> reg -> smem -> reg -> global
     QFT_KERNEL_TMA2 = 2,     // persistent: TMA tile load -> reg -> smem -> reg -> global, packed FP32x2
+    QFT_KERNEL_TMA2PP = 3,   // tma2 on 2^14 tiles: two thread groups ping-pong on one exchange buffer
 };
 
 // QFT_KERNEL_TMA2 only.  Every shared-memory byte offset is a GF(2)-linear function of the thread
@@ -56,6 +59,7 @@ struct QftTma2Desc {
     int8_t t1_lo, t2_lo;                    // lowest logical qubit of group 1 / group 2
     int8_t r1, r2;
     int8_t tma_lo[5], tma_len[5], tma_box[5];  // tensor-map dims: address bits [lo, lo+len), box 2^box
+    int8_t pp;                                 // ping-pong variant: thread bit 8 = group bit, swizzled landing
     int8_t land_addr[16];                      // landing-index bit j of the shared-memory tile <-> address bit
 };
 

@@ -334,11 +334,12 @@ def main():
     achieved = bytes_per_launch / (dom_ms * 1e-3) / 1e9
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            tj = json.load(fh)
-        ent = tj.get(f"n{n}", {}).get(dom)
-        if ent:
-            traffic = float(ent["dram_bytes_per_launch"])
+        # measured DRAM bytes per launch of the dominant kernel, from the committed ncu --set full capture
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+            for row in fh:
+                f = [v.strip() for v in row.split(",")]
+                if len(f) >= 3 and f[0] == str(n) and f[1] == dom:
+                    traffic = float(f[2])
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",

@@ -24,6 +24,7 @@ namespace {
 struct PassSpec {
     std::vector<int> window;                 // logical qubits, descending; empty = permutation only
     std::vector<int> F;                      // tile address bits
+    std::vector<int> Fbase;                  // F before the passive extras were added
     std::vector<std::pair<int, int>> moves;  // in-tile: data on address first goes to address second
     std::vector<std::pair<int, int>> swaps;  // non-tile address pairs (lo, hi) that trade places
 };
@@ -31,6 +32,8 @@ struct PassSpec {
 int ilog2_ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 void add_extras(PassSpec& ps, int n, int ftarget) {
+    if (ps.Fbase.empty()) ps.Fbase = ps.F;
+    else ps.F = ps.Fbase;
     std::set<int> used(ps.F.begin(), ps.F.end());
     std::set<int> sw;
     for (auto& s : ps.swaps) { sw.insert(s.first); sw.insert(s.second); }
@@ -533,8 +536,10 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         *err = "invalid argument";
         return 1;
     }
-    int fmax = prm.tile_bits ? prm.tile_bits : 13;
-    int l = prm.hub_bits ? prm.hub_bits : 3;
+    // defaults from the B200 sweep (profiles/r01_tile_hub_sweep.md): 128-byte granules (hub 4) as soon as
+    // the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit windows pay off
+    int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : 13);
+    int l = prm.hub_bits ? prm.hub_bits : (n >= 20 ? 4 : 3);
     if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 5 || l >= fmax) {
         *err = "unsupported tile_bits / hub_bits";
         return 2;
@@ -563,7 +568,33 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     int wmaxseen = 0;
     for (auto& ps : specs) {
         QftPassDesc d;
-        if (!lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u), (prm.flags & 8u) != 0, qubit_at, &d, err)) return 5;
+        {
+            // the passive extra tile bits are optional: if the full tile does not fit the TMA kernel
+            // (too many tensor-map dims, too many low in-tile qubits), try smaller tiles
+            const bool want_tma = !(prm.flags & 5u) && ps.window.size() >= 7;
+            bool done = false;
+            if (want_tma && !ps.Fbase.empty()) {
+                for (int ft = (int)ps.F.size(); ft >= 12 && ft >= (int)ps.Fbase.size() && !done; --ft) {
+                    PassSpec trial = ps;
+                    add_extras(trial, n, ft);
+                    if ((int)trial.F.size() != ft) continue;
+                    std::vector<int> qa = qubit_at;
+                    QftPassDesc dt;
+                    std::string e2;
+                    if (lower_pass(trial, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), true,
+                                   (prm.flags & 8u) != 0, qa, &dt, &e2) &&
+                        (dt.kernel == QFT_KERNEL_TMA2 || dt.kernel == QFT_KERNEL_TMA2PP)) {
+                        d = dt;
+                        qubit_at = qa;
+                        done = true;
+                    }
+                }
+            }
+            if (!done &&
+                !lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u),
+                            (prm.flags & 8u) != 0, qubit_at, &d, err))
+                return 5;
+        }
         wmaxseen = std::max(wmaxseen, (int)ps.window.size());
         out->passes.push_back(d);
     }

@@ -254,6 +254,9 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         a = b;
     }
     if (dims.size() > 5 || dims[0].box < 1 || dims[0].cls == 2) return;
+    // (only needed when the hub alone does not fill the four lowest landing bits; otherwise keep the
+    // natural, address-ascending order)
+    if (dims[0].box < 4)
     std::stable_sort(dims.begin() + 1, dims.end(), [](const Dim& x, const Dim& y) {
         const int kx = x.cls == 2 ? 1 : 0, ky = y.cls == 2 ? 1 : 0;
         return kx < ky;

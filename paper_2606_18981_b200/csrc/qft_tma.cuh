@@ -7,10 +7,11 @@
 //            no thread computes a global load address, and the load of tile i+1 is issued as soon as
 //            the buffer is free, so it is in flight while tile i is still being transformed and stored;
 //   step 1 : each thread takes the 32 amplitudes of its radix-2^R1 butterflies, applies H and the
-//            controlled-R_m onto the window's R1 highest qubits with packed FP32x2
-//            arithmetic, multiplies by the phase that group 2's qubits contribute,
-//            and writes to an XOR-swizzled exchange layout;
-//   step 2 : the same for the window's R2 lower qubits, then one more phase per amplitude: the product
+//            controlled-R_m among the window's R1 highest qubits with packed FP32x2
+//            arithmetic and writes to an XOR-swizzled exchange layout;
+//   step 2 : first the phases group 2's qubits contribute to group 1 (diagonal, so they
+//            may wait until after the exchange), then the same butterflies for the window's R2 lower
+//            qubits, then one more phase per amplitude: the product
 //            of every controlled-R_m from a qubit *below* the window onto any of the window's qubits.
 //            For group 1 that phase was deferred: it is diagonal in bits step 2 does not touch, so it
 //            commutes with step 2 and the two multiplications merge into one;
@@ -124,7 +125,6 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     uint32_t off1_ld = xor_cols(t.s1_tid_ld, tid, LT);
     uint32_t off1_mid = xor_cols(t.s1_tid_mid, tid, LT);
     uint32_t off2_mid = xor_cols(t.s2_tid_mid, tid, LT);
-    const uint32_t key1 = xor_cols(t.s1_tid_key, tid, LT);
     const uint32_t key2 = xor_cols(t.s2_tid_key, tid, LT);
     uint64_t st_thread = 0;
     for (int j = 0; j < LT; ++j)
@@ -146,11 +146,16 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         mbar_init(mbar, 1);
         fence_proxy_async();
     }
-    // mid bases: midW[v][i] = product of the controlled-R_m from group 2's qubits (value v) onto
-    // group 1's i-th qubit
-    for (uint32_t i = tid; i < 32u * R1; i += NT) {
-        const uint32_t v = i / R1, q = i % R1;
-        midW[v * kMidStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32((uint64_t)v << t.t2_lo, t.t1_lo + (int)q, k));
+    // mid bases: midW[u1][b] = the phase that group 2's b-th qubit (when set) contributes to an amplitude
+    // whose group-1 frequency bits are u1: the product over the set bits i of u1 of the controlled-R_m
+    // from that qubit onto group 1's i-th qubit (phases add exactly as 32-bit fractions of a turn)
+    for (uint32_t i = tid; i < 32u * R2; i += NT) {
+        const uint32_t u1 = i / R2, b = i % R2;
+        uint32_t ph = 0;
+#pragma unroll
+        for (int q = 0; q < R1; ++q)
+            if ((u1 >> q) & 1u) ph += qftp::cr_phase_u32(1ull << (t.t2_lo + (int)b), t.t1_lo + q, k);
+        midW[u1 * kMidStride + b] = qftp::cis_fwd_u32(ph);
     }
     __syncthreads();
 
@@ -233,23 +238,6 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
             for (int B = 0; B < 32; ++B) x[B].y = -x[B].y;
         }
         qftp::dif_group<5, R1, KC>(x);
-        {
-            constexpr int NB1 = 1 << (5 - R1);
-            float2 W1[NB1][5];
-            float2 one[NB1];
-#pragma unroll
-            for (int bt = 0; bt < NB1; ++bt) {
-                uint32_t kk = key1;
-#pragma unroll
-                for (int i = 0; i < 5 - R1; ++i)
-                    if (bt & (1 << i)) kk ^= t.s1_reg_key[R1 + i];
-                const float2* row = midW + (kk & 31u) * kMidStride;
-#pragma unroll
-                for (int i = 0; i < R1; ++i) W1[bt][i] = row[i];
-                one[bt] = make_float2(1.f, 0.f);
-            }
-            BatchApply<R1, 0, NB1, false>::run(x, W1, one);
-        }
 #define QFT_ST1(B) sts64(smem_raw, off1_mid ^ reg_off<B>(c1mid), x[B]);
         QFT_ALL32(QFT_ST1)
 #undef QFT_ST1
@@ -267,6 +255,25 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
             tma_load_5d(smem_raw, &tmap, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
         }
 
+        {
+            // the phases group 2's qubits put on group 1's frequency bits, applied here, after
+            // the exchange, so that the next tile's load is issued before this arithmetic rather than after
+            constexpr int NBM = 1 << (5 - R2);
+            float2 WM[NBM][5];
+            float2 one[NBM];
+#pragma unroll
+            for (int bt = 0; bt < NBM; ++bt) {
+                uint32_t kk = key2;
+#pragma unroll
+                for (int i = 0; i < 5 - R2; ++i)
+                    if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
+                const float2* row = midW + (kk & 31u) * kMidStride;
+#pragma unroll
+                for (int i = 0; i < R2; ++i) WM[bt][i] = row[i];
+                one[bt] = make_float2(1.f, 0.f);
+            }
+            BatchApply<R2, 0, NBM, false>::run(x, WM, one);
+        }
         qftp::dif_group<5, R2, KC>(x);
         if (has_end) {
             constexpr int NB2 = 1 << (5 - R2);

@@ -84,6 +84,17 @@ qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, i
                              qft_norm_t normalisation);
 
 /*
+ * qft_plan_create_batched -- plan for 2^log2_batch independent n_qubits-qubit transforms stored back to
+ * back: device_state of qft_execute is float2[2^(n_qubits + log2_batch)], state b occupying elements
+ * [b 2^n, (b+1) 2^n); every state gets the transform of qft_plan_create, in place, in the same launches.
+ * This is SURVEY.md section 8(f1): the paper's measured sizes (n = 12 ... 22) cannot fill a
+ * B200 one at a time.  n_qubits + log2_batch <= 34; log2_batch = 0 is qft_plan_create.  Other arguments,
+ * errors and ownership as for qft_plan_create.
+ */
+qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_batch, int aqft_cutoff_k,
+                                     int max_fused_qubits, int sign, qft_norm_t normalisation);
+
+/*
  * qft_plan_create_tuned -- as qft_plan_create, with the layout knobs exposed for
  * benchmarking: tile_bits (log2 amplitudes per tile, 0 = default), hub_bits
  * (log2 amplitudes per contiguous granule, 0 = default), flags (QFT_FLAG_*).

@@ -25,7 +25,7 @@ QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_PINGPONG = 1
 QFT_MAX_QUBITS = 34
 
 EXPORTS = [
-    "qft_plan_create", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
+    "qft_plan_create", "qft_plan_create_batched", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
     "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
 ]
@@ -59,6 +59,8 @@ def load() -> ctypes.CDLL:
     vp, ci = ctypes.c_void_p, ctypes.c_int
     L.qft_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci]
     L.qft_plan_create.restype = ci
+    L.qft_plan_create_batched.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ci]
+    L.qft_plan_create_batched.restype = ci
     L.qft_plan_create_tuned.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ci, ci, ctypes.c_uint]
     L.qft_plan_create_tuned.restype = ci
     L.qft_execute.argtypes = [vp, vp, vp]
@@ -104,6 +106,16 @@ def qft_plan_create(n_qubits: int, aqft_cutoff_k: int, max_fused_qubits: int = 1
     st = load().qft_plan_create(ctypes.byref(h), n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation)
     if st != QFT_OK:
         raise QftError(st, "qft_plan_create")
+    return h.value
+
+
+def qft_plan_create_batched(n_qubits: int, log2_batch: int, aqft_cutoff_k: int, max_fused_qubits: int = 13,
+                            sign: int = -1, normalisation: int = QFT_NORM_UNITARY) -> int:
+    h = ctypes.c_void_p()
+    st = load().qft_plan_create_batched(ctypes.byref(h), n_qubits, log2_batch, aqft_cutoff_k, max_fused_qubits, sign,
+                                        normalisation)
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_create_batched")
     return h.value
 
 
@@ -174,12 +186,19 @@ class Plan:
     """RAII wrapper: Plan(n, k).execute(tensor) transforms a CUDA complex64 tensor in place."""
 
     def __init__(self, n_qubits: int, aqft_cutoff_k: int | None = None, max_fused_qubits: int = 13, sign: int = -1,
-                 normalisation: int = QFT_NORM_UNITARY, tile_bits: int = 0, hub_bits: int = 0, flags: int = 0):
+                 normalisation: int = QFT_NORM_UNITARY, tile_bits: int = 0, hub_bits: int = 0, flags: int = 0,
+                 log2_batch: int = 0):
         if aqft_cutoff_k is None:
             aqft_cutoff_k = n_qubits
-        self.n = n_qubits
-        self.handle = qft_plan_create_tuned(n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation,
-                                            tile_bits, hub_bits, flags)
+        self.n = n_qubits + log2_batch  # address bits of the state this plan transforms
+        if log2_batch:
+            if tile_bits or hub_bits or flags:
+                raise ValueError("the tuning knobs are not available for batched plans")
+            self.handle = qft_plan_create_batched(n_qubits, log2_batch, aqft_cutoff_k, max_fused_qubits, sign,
+                                                  normalisation)
+        else:
+            self.handle = qft_plan_create_tuned(n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation,
+                                                tile_bits, hub_bits, flags)
 
     def execute(self, state, stream: int | None = None) -> None:
         """state: torch complex64 CUDA tensor of 2^n elements (contiguous).  In place, asynchronous."""

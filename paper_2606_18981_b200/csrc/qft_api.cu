@@ -59,6 +59,38 @@ qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutof
     return QFT_OK;
 }
 
+qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_batch, int aqft_cutoff_k,
+                                     int max_fused_qubits, int sign, qft_norm_t normalisation) {
+    if (!out) return QFT_ERR_INVALID_ARG;
+    QftPlanParams prm;
+    prm.n = n_qubits;
+    prm.batch_bits = log2_batch;
+    prm.k = aqft_cutoff_k;
+    prm.max_fused = max_fused_qubits;
+    prm.sign = sign;
+    prm.norm = (int)normalisation;
+    qft_plan_s* p = new (std::nothrow) qft_plan_s();
+    if (!p) return QFT_ERR_ALLOC;
+    std::string err;
+    int rc;
+    try {
+        rc = qft_build_plan(prm, &p->host, &err);
+    } catch (const std::bad_alloc&) {
+        delete p;
+        return QFT_ERR_ALLOC;
+    } catch (...) {
+        delete p;
+        return QFT_ERR_INTERNAL;
+    }
+    if (rc != 0) {
+        delete p;
+        g_cuda_err = err;
+        return (qft_status_t)rc;
+    }
+    *out = p;
+    return QFT_OK;
+}
+
 qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                              qft_norm_t normalisation) {
     return qft_plan_create_tuned(out, n_qubits, aqft_cutoff_k, max_fused_qubits, sign, normalisation, 0, 0, 0u);
@@ -86,7 +118,7 @@ qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_stat
 
 qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream) {
     if (!plan || !host_state) return QFT_ERR_INVALID_ARG;
-    const size_t bytes = (size_t)8 << plan->host.prm.n;
+    const size_t bytes = (size_t)8 << (plan->host.prm.n + plan->host.prm.batch_bits);
     cudaStream_t s = (cudaStream_t)stream;
     if (!plan->dev_buf) {
         cudaError_t e = cudaMalloc(&plan->dev_buf, bytes);

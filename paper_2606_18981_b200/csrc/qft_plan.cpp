@@ -533,7 +533,12 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
 }  // namespace
 
 int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err) {
-    const int n = prm.n;
+    const int n = prm.n;                  // qubits of one transform
+    const int na = prm.n + prm.batch_bits;  // address bits of the whole (batched) state
+    if (prm.batch_bits < 0 || na > 34) {
+        *err = "invalid argument";
+        return 1;
+    }
     if (n < 1 || n > 34 || prm.k < 0 || prm.max_fused < 1 || (prm.sign != 1 && prm.sign != -1) || prm.norm < 0 ||
         prm.norm > 2) {
         *err = "invalid argument";
@@ -542,12 +547,12 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     // defaults from the B200 sweep (profiles/r01_tile_hub_sweep.md): 128-byte granules (hub 4) as soon as
     // the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit windows pay off
     int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : 13);
-    int l = prm.hub_bits ? prm.hub_bits : (n >= 20 ? 4 : 3);
+    int l = prm.hub_bits ? prm.hub_bits : (na >= 20 ? 4 : 3);
     if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 5 || l >= fmax) {
         *err = "unsupported tile_bits / hub_bits";
         return 2;
     }
-    if (n - std::min(fmax, n) > 30) { *err = "tile_bits too small for this n"; return 2; }
+    if (na - std::min(fmax, na) > 30) { *err = "tile_bits too small for this n"; return 2; }
     out->prm = prm;
     out->k_eff = std::min(prm.k, n);
     out->tile_bits = fmax;
@@ -566,8 +571,12 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         specs.clear();
         build_unfolded(n, prm.max_fused, fmax, l, &specs);
     }
-    std::vector<int> qubit_at(n);
-    for (int a = 0; a < n; ++a) qubit_at[a] = a;
+    // batched plans: the batch index occupies address bits [n, na); they hold no qubit (ids >= n stand for
+    // "never processed"), never move, and serve as tile-index bits or passive in-tile bits
+    std::vector<int> qubit_at(na);
+    for (int a = 0; a < na; ++a) qubit_at[a] = a;
+    if (na > n)
+        for (auto& ps : specs) add_extras(ps, na, std::min(fmax, na));
     int wmaxseen = 0;
     for (auto& ps : specs) {
         QftPassDesc d;
@@ -579,12 +588,12 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
             if (want_tma && !ps.Fbase.empty()) {
                 for (int ft = (int)ps.F.size(); ft >= 12 && ft >= (int)ps.Fbase.size() && !done; --ft) {
                     PassSpec trial = ps;
-                    add_extras(trial, n, ft);
+                    add_extras(trial, na, ft);
                     if ((int)trial.F.size() != ft) continue;
                     std::vector<int> qa = qubit_at;
                     QftPassDesc dt;
                     std::string e2;
-                    if (lower_pass(trial, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), true,
+                    if (lower_pass(trial, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), true,
                                    (prm.flags & 8u) != 0, qa, &dt, &e2) &&
                         (dt.kernel == QFT_KERNEL_TMA2 || dt.kernel == QFT_KERNEL_TMA2PP)) {
                         d = dt;
@@ -594,7 +603,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
                 }
             }
             if (!done &&
-                !lower_pass(ps, n, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u),
+                !lower_pass(ps, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u),
                             (prm.flags & 8u) != 0, qubit_at, &d, err))
                 return 5;
         }
@@ -619,10 +628,11 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
 
 // Independent re-derivation from the descriptors alone.
 int qft_check_plan(const QftHostPlan& plan, std::string* err) {
-    const int n = plan.prm.n;
+    const int nq = plan.prm.n;                      // qubits of one transform
+    const int n = plan.prm.n + plan.prm.batch_bits;  // address bits
     std::vector<int> qubit_at(n);
     for (int a = 0; a < n; ++a) qubit_at[a] = a;
-    int next_qubit = n - 1;
+    int next_qubit = nq - 1;
     char buf[256];
     int pi = 0;
     int nscaled = 0;
@@ -841,7 +851,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
     }
     if (next_qubit != -1) { *err = "self-check: not every qubit was processed"; return 5; }
     for (int a = 0; a < n; ++a)
-        if (qubit_at[a] != n - 1 - a) { *err = "self-check: final layout is not the bit reversal"; return 5; }
+        if (qubit_at[a] != (a < nq ? nq - 1 - a : a)) { *err = "self-check: final layout is not the bit reversal"; return 5; }
     const bool want_scale = plan.prm.norm != 1;
     if ((want_scale && nscaled != 1) || (!want_scale && nscaled != 0)) { *err = "self-check: scale"; return 5; }
     return 0;
@@ -849,7 +859,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
 
 std::string qft_describe_plan(const QftHostPlan& plan) {
     std::ostringstream o;
-    o << "{\"n\":" << plan.prm.n << ",\"k\":" << plan.k_eff << ",\"sign\":" << plan.prm.sign
+    o << "{\"n\":" << plan.prm.n << ",\"batch_bits\":" << plan.prm.batch_bits << ",\"k\":" << plan.k_eff << ",\"sign\":" << plan.prm.sign
       << ",\"norm\":" << plan.prm.norm << ",\"max_fused_qubits\":" << plan.prm.max_fused
       << ",\"tile_bits\":" << plan.tile_bits << ",\"hub_bits\":" << plan.hub_bits
       << ",\"folded\":" << (plan.folded ? "true" : "false") << ",\"n_h\":" << plan.n_h << ",\"n_cr\":" << plan.n_cr
@@ -880,7 +890,7 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
         o << "],\"pair_swaps\":[";
         for (int p = 0; p < d.npair; ++p)
             o << (p ? "," : "") << "[" << (int)d.tile_addr[p] << "," << (int)d.tile_addr[d.npair + p] << "]";
-        o << "],\"scale\":" << d.scale << ",\"bytes\":" << (16.0 * std::ldexp(1.0, plan.prm.n)) << "}";
+        o << "],\"scale\":" << d.scale << ",\"bytes\":" << (16.0 * std::ldexp(1.0, plan.prm.n + plan.prm.batch_bits)) << "}";
     }
     o << "]}";
     return o.str();

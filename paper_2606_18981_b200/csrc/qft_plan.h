@@ -102,6 +102,7 @@ struct QftPassDesc {
 
 struct QftPlanParams {
     int n = 0;
+    int batch_bits = 0;  // log2 of the number of independent states stored back to back
     int k = 0;
     int max_fused = 0;
     int sign = -1;

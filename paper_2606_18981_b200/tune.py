@@ -23,13 +23,16 @@ def main() -> int:
     ap.add_argument("--hub-bits", type=int, default=0)
     ap.add_argument("--flags", type=int, default=0)
     ap.add_argument("--max-fused", type=int, default=13)
+    ap.add_argument("--log2-batch", type=int, default=0, help="2^b independent transforms back to back")
     ap.add_argument("--reps", type=int, default=2)
     ap.add_argument("--no-time", action="store_true")
     a = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("needs a CUDA device")
     n = a.n
-    plan = qft.Plan(n, n if a.k is None else a.k, a.max_fused, -1, qft.QFT_NORM_UNITARY, a.tile_bits, a.hub_bits, a.flags)
+    plan = qft.Plan(n, n if a.k is None else a.k, a.max_fused, -1, qft.QFT_NORM_UNITARY, a.tile_bits, a.hub_bits, a.flags,
+                    a.log2_batch)
+    n = a.n + a.log2_batch  # address bits from here on
     st = torch.empty(1 << n, dtype=torch.complex64, device="cuda")
     torch.view_as_real(st).normal_()
     st.mul_(2.0 ** (-(n + 1) / 2))
@@ -58,7 +61,7 @@ def main() -> int:
     e1.record()
     torch.cuda.synchronize()
     d = plan.describe()
-    print(json.dumps({"n": n, "k": d["k"], "tile_bits": d["tile_bits"], "hub_bits": d["hub_bits"], "passes": npass,
+    print(json.dumps({"n": d["n"], "batch_bits": d["batch_bits"], "k": d["k"], "tile_bits": d["tile_bits"], "hub_bits": d["hub_bits"], "passes": npass,
                       "kernels": [p["kernel"] for p in d["passes"]], "steps": [p["steps"] for p in d["passes"]],
                       "pass_ms": [round(v, 3) for v in acc], "execute_ms": round(e0.elapsed_time(e1) / reps, 3),
                       "gbs_per_pass": [round(16.0 * (1 << n) / v / 1e6) for v in acc]}))

@@ -249,10 +249,11 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     const bool pp = d.kernel == QFT_KERNEL_TMA2PP;
-    const size_t smem = pp ? (size_t)QFT_TMA2PP_SMEM_BYTES : ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES;
+    const size_t smem = pp ? (size_t)QFT_TMA2PP_SMEM_BYTES : ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb);
     cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const int per_sm = d.f == 13 ? 2 : (d.f == 12 ? 4 : 1);
+    int per_sm = d.f == 13 ? 2 : (d.f == 12 ? 4 : 1);
+    while (per_sm > 1 && per_sm * (smem + 1024) > 227 * 1024) --per_sm;
     const unsigned csz = d.npair ? 2u : 1u;
     unsigned long long ntiles = 1ull << d.ntile;
     unsigned long long grid = (unsigned long long)sm_count() * per_sm;

@@ -15,6 +15,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <set>
 #include <sstream>
@@ -143,8 +144,9 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) 
     return true;
 }
 
-std::vector<int> step_sizes(int w) {
+std::vector<int> step_sizes(int w, bool force2 = false) {
     if (w <= 0) return {};
+    if (force2 && (w == 4 || w == 5)) return split_balanced(w, 2);  // two register groups for the TMA kernel
     const int g = ilog2_ceil_div(w, QFT_MAX_RADIX_BITS);
     return split_balanced(w, g);  // larger groups first
 }
@@ -208,17 +210,26 @@ bool solve_swizzle(const int (&L1)[4], const int (&L2)[4], int f, uint8_t (&lowm
 }
 
 // Fills d->tma and sets d->kernel = QFT_KERNEL_TMA2 when the pass fits the kernel's shape.
+// QFT_PLAN_DEBUG=1 in the environment prints why a pass was not given to the TMA kernel
+#define QFT_REJECT(code)                                                                        \
+    do {                                                                                        \
+        if (getenv("QFT_PLAN_DEBUG")) fprintf(stderr, "lower_tma2(pp=%d): reject at #%d (f=%d r=%d+%d)\n", (int)pp, code, d->f, d->steps[0].r, d->steps[1].r); \
+        return;                                                                                 \
+    } while (0)
 void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     const int f = d->f;
-    if (pp && f != 14) return;
+    if (pp && f != 14) QFT_REJECT(1);
     const QftStep s1 = d->steps[0], s2 = d->steps[1];
     const int r1 = s1.r, r2 = s2.r;
-    if (f < 12 || f > 14) return;
-    if (!((r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3))) return;
-    if (s1.a != s2.a + r2) return;  // the window is one run of canonical bits
+    if (f < 12 || f > 14) QFT_REJECT(2);
+    if (!((r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3) ||
+          (r1 == 3 && r2 == 3) || (r1 == 3 && r2 == 2) || (r1 == 2 && r2 == 2)))
+        QFT_REJECT(3);
+    if (pp && r1 + r2 < 7) QFT_REJECT(4);
+    if (s1.a != s2.a + r2) QFT_REJECT(5);  // the window is one run of canonical bits
     const int eb = s2.a;            // canonical bits below the window
-    if (eb > 5) return;
-    if (n - f < 1) return;
+    if (eb > 7 || (pp && eb > 5)) QFT_REJECT(6);
+    if (n - f < 1) QFT_REJECT(7);
     (void)hub;
     QftTma2Desc t;
     std::memset(&t, 0, sizeof t);
@@ -231,7 +242,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         canon_at_load[d->F[j]] = d->ld_canon[j];
         st_idx_of_canon[d->st_canon[j]] = j;
     }
-    if (!inF[0] || !inF[1]) return;  // the innermost box dimension must span >= 16 bytes
+    if (!inF[0] || !inF[1]) QFT_REJECT(8);  // the innermost box dimension must span >= 16 bytes
     // ---- tensor-map dims: runs of address bits inside / outside F.  In-tile runs are cut where the
     // group membership changes and to <= 8 bits (box <= 256); the run that starts at address bit 0 is
     // dimension 0 (TMA's contiguous one).  The box lands in shared memory dimension by dimension, so
@@ -239,7 +250,10 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     // the four lowest landing-index bits (conflict-free reads by lanes that run along the low bits).
     struct Dim { int lo, len, box, cls; };
     std::vector<Dim> dims;
-    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return in1(c) ? 2 : 0; };
+    int hubrun = 0;
+    while (hubrun < n && inF[hubrun]) ++hubrun;
+    // runs are cut where group-1 membership changes only if the dims will have to be reordered
+    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return (hubrun < 4 && in1(c)) ? 2 : 0; };
     int a = 0;
     while (a < n) {
         int b = a + 1;
@@ -253,7 +267,8 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         }
         a = b;
     }
-    if (dims.size() > 5 || dims[0].box < 1 || dims[0].cls == 2) return;
+    if (dims.size() > 5 || dims[0].box < 1 || dims[0].cls == 2) QFT_REJECT(9);
+    if (hubrun >= 4 && dims[0].box < 4) QFT_REJECT(10);
     // (only needed when the hub alone does not fill the four lowest landing bits; otherwise keep the
     // natural, address-ascending order)
     if (dims[0].box < 4)
@@ -274,16 +289,16 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
             ++nland;
         }
     }
-    if (nland != f) return;
+    if (nland != f) QFT_REJECT(11);
     // ---- threads and registers of the two steps (canonical bits) ----
     // step 1: register bits = group 1 (+ batch bits: the highest landing bits outside the group);
     // thread bits = the remaining landing bits, ascending, so lanes read consecutive shared memory
     std::vector<int> reg1, thr1, reg2, thr2;
     int gcan = -1;  // ping-pong: the canonical bit that splits the tile between the two thread groups
     if (pp) {
-        if (dims[0].box != 4) return;
+        if (dims[0].box != 4) QFT_REJECT(12);
         gcan = canon_at_load[t.land_addr[3]];
-        if (in1(gcan) || in2(gcan)) return;
+        if (in1(gcan) || in2(gcan)) QFT_REJECT(13);
     }
     for (int b = 0; b < r1; ++b) reg1.push_back(s1.a + b);
     {
@@ -299,7 +314,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
             // swizzle a half-warp then covers all 32 banks; the group bit is the top thread bit
             const int c6 = canon_at_load[t.land_addr[6]];
             auto it = std::find(thr1.begin(), thr1.end(), c6);
-            if (it == thr1.end() || (it - thr1.begin()) < 3) return;
+            if (it == thr1.end() || (it - thr1.begin()) < 3) QFT_REJECT(14);
             thr1.erase(it);
             thr1.insert(thr1.begin() + 3, c6);
             thr1.push_back(gcan);
@@ -316,25 +331,25 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         thr2 = rest;
         if (pp) thr2.push_back(gcan);
     }
-    if ((int)thr1.size() != lt || (int)thr2.size() != lt) return;
+    if ((int)thr1.size() != lt || (int)thr2.size() != lt) QFT_REJECT(15);
     if (pp) {
         for (int j = 0; j < 3; ++j)
-            if (land_idx_of_canon[thr1[j]] != j || st_idx_of_canon[thr2[j]] != j) return;
-        for (int c : reg1) if (c == gcan) return;
-        for (int c : reg2) if (c == gcan) return;
+            if (land_idx_of_canon[thr1[j]] != j || st_idx_of_canon[thr2[j]] != j) QFT_REJECT(16);
+        for (int c : reg1) if (c == gcan) QFT_REJECT(17);
+        for (int c : reg2) if (c == gcan) QFT_REJECT(18);
     } else {
         for (int j = 0; j < 4; ++j)
-            if (land_idx_of_canon[thr1[j]] != j) return;
-        const int hubrun = dims[0].box;
-        for (int j = 0; j < std::min(hubrun, 4); ++j)
-            if (st_idx_of_canon[thr2[j]] != j) return;
+            if (land_idx_of_canon[thr1[j]] != j) QFT_REJECT(19);
+        const int hubrun0 = dims[0].box;
+        for (int j = 0; j < std::min(hubrun0, 4); ++j)
+            if (st_idx_of_canon[thr2[j]] != j) QFT_REJECT(20);
     }
     // exchange layout: canonical index (ping-pong: with the group bit squeezed out) XOR-swizzled
     auto xpos = [&](int c) { return (gcan >= 0 && c > gcan) ? c - 1 : c; };
     int L1[4], L2[4];
     for (int j = 0; j < 4; ++j) { L1[j] = xpos(thr1[j]); L2[j] = xpos(thr2[j]); }
     uint8_t lowmask[16];
-    if (!solve_swizzle(L1, L2, f, lowmask)) return;
+    if (!solve_swizzle(L1, L2, f, lowmask)) QFT_REJECT(21);
     auto midcol = [&](int c) -> uint32_t {
         if (c == gcan) return 0u;
         const int p = xpos(c);
@@ -385,9 +400,10 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     d->log2_threads = lt;
 }
 
+#undef QFT_REJECT
 // Turn a PassSpec into the kernel descriptor given the current layout; updates qubit_at.
 bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma, bool allow_pp,
-                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err) {
+                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err, bool force2 = false) {
     std::memset(d, 0, sizeof(*d));
     const int f = (int)ps.F.size();
     if (f > QFT_MAX_TILE_BITS || n - f > QFT_MAX_TILEIDX_BITS) { *err = "tile too large"; return false; }
@@ -451,7 +467,7 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
         }
         d->win_lo = ps.window[w - 1];
         int t = ps.window[0];
-        for (int r : step_sizes(w)) {
+        for (int r : step_sizes(w, force2)) {
             QftStep& st = d->steps[d->nsteps++];
             st.r = (int8_t)r;
             st.t_hi = (int8_t)t;
@@ -569,7 +585,9 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     if (!(prm.flags & 2u)) out->folded = build_folded(n, prm.max_fused, fmax, l, &specs);
     if (!out->folded) {
         specs.clear();
-        build_unfolded(n, prm.max_fused, fmax, l, &specs);
+        // batched transforms that fit one tile: two two-step passes (TMA kernel) beat one three-step pass
+        const int wcap = (prm.batch_bits > 0 && n > 10 && n <= fmax) ? std::min(prm.max_fused, (n + 1) / 2) : prm.max_fused;
+        build_unfolded(n, wcap, fmax, l, &specs);
     }
     // batched plans: the batch index occupies address bits [n, na); they hold no qubit (ids >= n stand for
     // "never processed"), never move, and serve as tile-index bits or passive in-tile bits
@@ -583,7 +601,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         {
             // the passive extra tile bits are optional: if the full tile does not fit the TMA kernel
             // (too many tensor-map dims, too many low in-tile qubits), try smaller tiles
-            const bool want_tma = !(prm.flags & 5u) && ps.window.size() >= 7;
+            const bool want_tma = !(prm.flags & 5u) && ps.window.size() >= 4;
             bool done = false;
             if (want_tma && !ps.Fbase.empty()) {
                 for (int ft = (int)ps.F.size(); ft >= 12 && ft >= (int)ps.Fbase.size() && !done; --ft) {
@@ -594,7 +612,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
                     QftPassDesc dt;
                     std::string e2;
                     if (lower_pass(trial, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), true,
-                                   (prm.flags & 8u) != 0, qa, &dt, &e2) &&
+                                   (prm.flags & 8u) != 0, qa, &dt, &e2, true) &&
                         (dt.kernel == QFT_KERNEL_TMA2 || dt.kernel == QFT_KERNEL_TMA2PP)) {
                         d = dt;
                         qubit_at = qa;
@@ -742,7 +760,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                         uint32_t kb = key;
                         for (int b = s1.r; b < 5; ++b) if ((B >> b) & 1) kb ^= t.s1_reg_key[b];
                         if ((kb & 31u) != v) return fail("tma2: step 1 key (group 2 value)");
-                        if (((kb >> 8) & 31u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
+                        if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
                         for (int b = 0; b < s1.r; ++b) if (t.s1_reg_key[b]) return fail("tma2: group bit in key");
                     }
                     (void)kk;
@@ -803,7 +821,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     const uint32_t c = (uint32_t)mid_canon[gs];
                     if (((c >> s2.a) & ((1u << s2.r) - 1u)) != (uint32_t)(B & ((1 << s2.r) - 1))) return fail("tma2: step 2 register bits");
                     if ((kb & 31u) != ((c >> s1.a) & ((1u << s1.r) - 1u))) return fail("tma2: step 2 key (group 1 value)");
-                    if (((kb >> 8) & 31u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
+                    if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
                     // the element with canonical index c must land on store-order index st(c)
                     uint32_t want = 0;
                     for (int j = 0; j < f; ++j) if ((c >> d.st_canon[j]) & 1u) want |= 1u << j;
@@ -813,7 +831,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 }
             }
             for (int j = 0; j < (pp ? 3 : std::min<int>(t.tma_box[0], 4)) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
-            if (t.eb != s2.a || t.eb > 5) return fail("tma2: eb");
+            if (t.eb != s2.a || t.eb > 7) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
             // tensor-map dims partition the address bits; box bits are exactly F; dim 0 starts at bit 0

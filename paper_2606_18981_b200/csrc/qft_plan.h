@@ -27,7 +27,7 @@
 #define QFT_TMA2_END_STRIDE 16  // float2 per row (R1 + R2 <= 10 used)
 // QFT_KERNEL_TMA2PP: 1 KB alignment slack + landing (2^14) + exchange (2^13) + mid + 4 end tables + mbarrier etc.
 #define QFT_TMA2PP_SMEM_BYTES (1024 + (8 << 14) + (8 << 13) + (32 * QFT_TMA2_MID_STRIDE + 4 * 32 * QFT_TMA2_END_STRIDE) * 8 + 8 + 48 + 8)
-#define QFT_TMA2_TABLE_BYTES ((32 * QFT_TMA2_MID_STRIDE + 2 * 32 * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)
+#define QFT_TMA2_TABLE_BYTES(eb) ((32 * QFT_TMA2_MID_STRIDE + 2 * ((eb) > 5 ? (1 << (eb)) : 32) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)
 
 struct QftStep {
     int8_t r;     // qubits in the group
@@ -51,11 +51,11 @@ struct QftTma2Desc {
     uint32_t s1_tid_ld[9], s1_reg_ld[5];    // step 1 read: the TMA landing layout (tile load order)
     uint32_t s1_tid_mid[9], s1_reg_mid[5];  // step 1 write: the swizzled exchange layout
     uint32_t s2_tid_mid[9], s2_reg_mid[5];  // step 2 read: the same layout seen from step 2's threads
-    uint16_t s1_tid_key[9], s1_reg_key[5];  // step 1 key: bits 0-4 = value of group 2's qubits, 8-12 = e
-    uint16_t s2_tid_key[9], s2_reg_key[5];  // step 2 key: bits 0-4 = value of group 1's qubits, 8-12 = e
+    uint16_t s1_tid_key[9], s1_reg_key[5];  // step 1 key: bits 0-4 = value of group 2's qubits, 8-14 = e
+    uint16_t s2_tid_key[9], s2_reg_key[5];  // step 2 key: bits 0-4 = value of group 1's qubits, 8-14 = e
     int8_t s2_tid_addr[9], s2_reg_addr[5];  // step 2 store: HBM address bit of each thread / register bit
-    int8_t eb;                              // in-tile logical qubits below the window (<= 5); e indexes them
-    int8_t e_log[5];                        // their logical ids, ascending
+    int8_t eb;                              // in-tile logical qubits below the window (<= 7); e indexes them
+    int8_t e_log[7];                        // their logical ids, ascending
     int8_t t1_lo, t2_lo;                    // lowest logical qubit of group 1 / group 2
     int8_t r1, r2;
     int8_t tma_lo[5], tma_len[5], tma_box[5];  // tensor-map dims: address bits [lo, lo+len), box 2^box

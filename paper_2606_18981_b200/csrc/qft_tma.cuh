@@ -115,9 +115,9 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     constexpr int F = LT + 5;
     constexpr int NT = 1 << LT;
     float2* midW = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F));
-    float2* endW = midW + 32 * kMidStride;
-    uint64_t* mbar = reinterpret_cast<uint64_t*>(endW + 2 * 32 * kEndStride);  // two end tables (by parity)
-    int* nextc = reinterpret_cast<int*>(mbar + 1);                              // next tile's TMA coordinates
+    uint64_t* mbar = reinterpret_cast<uint64_t*>(midW + 32 * kMidStride);
+    int* nextc = reinterpret_cast<int*>(mbar + 1);           // next tile's TMA coordinates (5 ints, padded to 6)
+    float2* endW = reinterpret_cast<float2*>(nextc + 6);     // two end tables (by parity) of max(32, 2^eb) rows
     const uint32_t tid = threadIdx.x;
     const QftTma2Desc& t = d.tma;
 
@@ -165,6 +165,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     const uint32_t nunits = (1u << d.ntile) / csz;
     const uint32_t ustride = gridDim.x / csz;
     const bool has_end = win_lo > 0;
+    const uint32_t end_rows = t.eb > 5 ? (1u << t.eb) : 32u;
 
     // tile index -> TMA coordinates (HBM address bits of the tile, cut into the tensor map's dims)
     auto coords_of = [&](uint32_t un, int (&c)[5]) {
@@ -188,7 +189,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     for (; unit < nunits; unit += ustride) {
         // ---- bookkeeping while the tile's load is in flight (few registers live here) ----
         uint64_t base_st = 0;
-        float2* endWp = endW + parity * (32 * kEndStride);
+        float2* endWp = endW + parity * (end_rows * kEndStride);
         {
             uint32_t ml, ms;
             decode_tile(unit * csz + rho, d.npair, &ml, &ms);
@@ -285,7 +286,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
 #pragma unroll
                 for (int i = 0; i < 5 - R2; ++i)
                     if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
-                const float2* row = endWp + ((kk >> 8) & 31u) * kEndStride;
+                const float2* row = endWp + ((kk >> 8) & 127u) * kEndStride;
 #pragma unroll
                 for (int i = 0; i < R2; ++i) W2[bt][i] = row[i];
                 float2 c = make_float2(d.scale, 0.f);

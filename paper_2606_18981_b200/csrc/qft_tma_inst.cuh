@@ -21,5 +21,8 @@ static tma2_kernel_t qft_pick_tma2_kc(int kc) {
         if (r1 == 5 && r2 == 4) return qft_pick_tma2_kc<5, 4, LT>(kc);    \
         if (r1 == 4 && r2 == 4) return qft_pick_tma2_kc<4, 4, LT>(kc);    \
         if (r1 == 4 && r2 == 3) return qft_pick_tma2_kc<4, 3, LT>(kc);    \
+        if (r1 == 3 && r2 == 3) return qft_pick_tma2_kc<3, 3, LT>(kc);    \
+        if (r1 == 3 && r2 == 2) return qft_pick_tma2_kc<3, 2, LT>(kc);    \
+        if (r1 == 2 && r2 == 2) return qft_pick_tma2_kc<2, 2, LT>(kc);    \
         return nullptr;                                                   \
     }

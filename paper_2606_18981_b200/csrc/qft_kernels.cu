@@ -169,6 +169,8 @@ static pass_kernel_t pick_kernel(const QftPassDesc& d) {
         QFT_PICK(4, 4)
         QFT_PICK(4, 3)
         QFT_PICK(3, 3)
+        QFT_PICK(3, 2)
+        QFT_PICK(2, 2)
 #undef QFT_PICK
     }
     return (pass_kernel_t)qftk::qft_tile_pass_generic;
@@ -176,7 +178,7 @@ static pass_kernel_t pick_kernel(const QftPassDesc& d) {
 
 bool qft_fused2_supported(int r1, int r2) {
     return (r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3) ||
-           (r1 == 3 && r2 == 3);
+           (r1 == 3 && r2 == 3) || (r1 == 3 && r2 == 2) || (r1 == 2 && r2 == 2);
 }
 
 // ---- QFT_KERNEL_TMA2 ---------------------------------------------------------------------------

@@ -250,10 +250,12 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     // the four lowest landing-index bits (conflict-free reads by lanes that run along the low bits).
     struct Dim { int lo, len, box, cls; };
     std::vector<Dim> dims;
-    int hubrun = 0;
-    while (hubrun < n && inF[hubrun]) ++hubrun;
-    // runs are cut where group-1 membership changes only if the dims will have to be reordered
-    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return (hubrun < 4 && in1(c)) ? 2 : 0; };
+    // the four lowest landing-index bits must not hold group-1 qubits; if the address-ascending order
+    // would put one there, runs are cut where group-1 membership changes and group 1's dims go last
+    bool need_reorder = false;
+    for (int j = 0; j < std::min(4, f); ++j)
+        if (in1(d->ld_canon[j])) need_reorder = true;
+    auto cls_of = [&](int a) { const int c = canon_at_load[a]; return (need_reorder && in1(c)) ? 2 : 0; };
     int a = 0;
     while (a < n) {
         int b = a + 1;
@@ -268,10 +270,9 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         a = b;
     }
     if (dims.size() > 5 || dims[0].box < 1 || dims[0].cls == 2) QFT_REJECT(9);
-    if (hubrun >= 4 && dims[0].box < 4) QFT_REJECT(10);
     // (only needed when the hub alone does not fill the four lowest landing bits; otherwise keep the
     // natural, address-ascending order)
-    if (dims[0].box < 4)
+    if (need_reorder)
     std::stable_sort(dims.begin() + 1, dims.end(), [](const Dim& x, const Dim& y) {
         const int kx = x.cls == 2 ? 1 : 0, ky = y.cls == 2 ? 1 : 0;
         return kx < ky;
@@ -340,8 +341,11 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     } else {
         for (int j = 0; j < 4; ++j)
             if (land_idx_of_canon[thr1[j]] != j) QFT_REJECT(19);
+        // store lanes: at least the three lowest hub bits (64-byte segments); a fourth hub bit that
+        // receives a group-2 qubit becomes a register bit (the two half lines leave the same warp a
+        // few instructions apart and merge in L2)
         const int hubrun0 = dims[0].box;
-        for (int j = 0; j < std::min(hubrun0, 4); ++j)
+        for (int j = 0; j < std::min(hubrun0, 3); ++j)
             if (st_idx_of_canon[thr2[j]] != j) QFT_REJECT(20);
     }
     // exchange layout: canonical index (ping-pong: with the group bit squeezed out) XOR-swizzled
@@ -620,6 +624,18 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
                     }
                 }
             }
+            if (!done && !(prm.flags & 1u) && (ps.window.size() == 4 || ps.window.size() == 5)) {
+                // a 4- or 5-qubit window as two register groups, so that the fused kernel can take it
+                std::vector<int> qa = qubit_at;
+                QftPassDesc dt;
+                std::string e2;
+                if (lower_pass(ps, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, true, false, false, qa, &dt, &e2, true) &&
+                    dt.kernel == QFT_KERNEL_FUSED2) {
+                    d = dt;
+                    qubit_at = qa;
+                    done = true;
+                }
+            }
             if (!done &&
                 !lower_pass(ps, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u),
                             (prm.flags & 8u) != 0, qubit_at, &d, err))
@@ -830,7 +846,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     seen_st[st_idx] = 1;
                 }
             }
-            for (int j = 0; j < (pp ? 3 : std::min<int>(t.tma_box[0], 4)) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
+            for (int j = 0; j < std::min<int>(t.tma_box[0], 3) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
             if (t.eb != s2.a || t.eb > 7) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");

@@ -256,6 +256,10 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     for (int j = 0; j < std::min(4, f); ++j)
         if (in1(d->ld_canon[j])) need_reorder = true;
     auto cls_of = [&](int a) { const int c = canon_at_load[a]; return (need_reorder && in1(c)) ? 2 : 0; };
+    // box dims: the runs of tile bits.  All tile-INDEX bits share ONE dimension of box 1 that spans from
+    // the lowest to the highest of them with the stride of the lowest: its coordinate is the tile's base
+    // address shifted down, and since a base address has zeros on every tile bit the sum
+    // coordinate x stride still lands on the right element (TMA checks bounds per dimension only).
     int a = 0;
     while (a < n) {
         int b = a + 1;
@@ -263,11 +267,15 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
             // dimension 0 may mix classes (it is the hub); the others may not
             while (b < n && inF[b] && b - a < ((pp && a == 0) ? 4 : 8) && (cls_of(b) == cls_of(a))) ++b;
             dims.push_back({a, b - a, b - a, cls_of(a)});
-        } else {
-            while (b < n && !inF[b] && b - a < 30) ++b;
-            dims.push_back({a, b - a, 0, -1});
         }
         a = b;
+    }
+    {
+        int tlo = -1, thi = -1;
+        for (int b = 0; b < n; ++b)
+            if (!inF[b]) { if (tlo < 0) tlo = b; thi = b; }
+        if (tlo < 0 || thi - tlo + 1 > 31) QFT_REJECT(22);
+        dims.push_back({tlo, thi - tlo + 1, 0, -1});
     }
     if (dims.size() > 5 || dims[0].box < 1 || dims[0].cls == 2) QFT_REJECT(9);
     // (only needed when the hub alone does not fill the four lowest landing bits; otherwise keep the
@@ -850,22 +858,30 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
             if (t.eb != s2.a || t.eb > 7) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
-            // tensor-map dims partition the address bits; box bits are exactly F; dim 0 starts at bit 0
-            int a = 0, boxbits = 0;
-            std::vector<int> covered(n + 1, 0);
+            // tensor-map dims: the box dims are disjoint runs that together are exactly F, dim 0 starts at
+            // bit 0; every tile-index bit lies inside the span of a box-1 dim (its coordinate is the tile's
+            // base address, which is zero on all tile bits, shifted down to the dim's lowest bit)
+            int boxbits = 0;
+            std::vector<int> covered(n + 1, 0), spanned(n + 1, 0);
             if (t.tma_lo[0] != 0) return fail("tma2: dimension 0 is not the contiguous one");
             for (int i = 0; i < 5; ++i) {
                 if (t.tma_box[i] != 0 && t.tma_box[i] != t.tma_len[i]) return fail("tma2: box");
-                if (t.tma_box[i] > 8 || t.tma_len[i] > 30) return fail("tma2: dim too large");
+                if (t.tma_box[i] > 8 || t.tma_len[i] > 31) return fail("tma2: dim too large");
                 for (int b = 0; b < t.tma_len[i]; ++b) {
                     const int bit = t.tma_lo[i] + b;
-                    if (bit < 0 || bit >= n || covered[bit]) return fail("tma2: tensor-map dims do not partition the address bits");
-                    covered[bit] = 1;
-                    if ((t.tma_box[i] != 0) != (inF[bit] != 0)) return fail("tma2: box bits are not the tile bits");
+                    if (bit < 0 || bit >= n) return fail("tma2: tensor-map dim outside the state");
+                    if (t.tma_box[i] != 0) {
+                        if (covered[bit] || !inF[bit]) return fail("tma2: box bits are not the tile bits");
+                        covered[bit] = 1;
+                    } else {
+                        spanned[bit] = 1;
+                    }
                 }
                 boxbits += t.tma_box[i];
-                a += t.tma_len[i];
             }
+            for (int bit = 0; bit < n; ++bit)
+                if (!inF[bit] && !spanned[bit]) return fail("tma2: a tile-index bit is outside the tensor map");
+            const int a = n;
             if (a != n || boxbits != f || t.tma_box[0] < 1) return fail("tma2: tensor map does not cover the state");
         }
         if (d.do_scale) ++nscaled;

@@ -45,6 +45,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", default="", help="comma list of extra n to time briefly, e.g. 20,22,26,33")
+    ap.add_argument("--batched", default="", help="comma list of n:log2_batch pairs to time briefly (batched plans), "
+                                                  "e.g. 10:18,16:12")
     return ap.parse_args()
 
 
@@ -139,13 +141,14 @@ def max_over_ranks(x: float, world: int, device) -> float:
     return float(t.item())
 
 
-def time_config(qft, torch, n, k, args, steps, warmup, per_pass=True):
+def time_config(qft, torch, n, k, args, steps, warmup, per_pass=True, log2_batch=0):
     """Device-resident timing of qft_execute on a fresh synthetic state; returns a dict."""
     import qft_inputs as qi
 
     dev = torch.device("cuda", torch.cuda.current_device())
     plan = qft.Plan(n, n if k is None else k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
-                    args.hub_bits, args.flags)
+                    args.hub_bits, args.flags, log2_batch)
+    n = n + log2_batch  # address bits of the state
     state = torch.empty(1 << n, dtype=torch.complex64, device=dev)
     if n <= 27:
         state.copy_(torch.from_numpy(qi.gaussian(n, 1)))
@@ -390,6 +393,24 @@ def main():
             del r
             torch.cuda.empty_cache()
 
+    batched = []
+    if args.batched and rank == 0:
+        try:
+            del state
+        except Exception:  # already released by the sweep
+            pass
+        torch.cuda.empty_cache()
+        for pair in [v for v in args.batched.split(",") if v]:
+            bn, bb = (int(v) for v in pair.split(":"))
+            r = time_config(qft, torch, bn, None, args, 10, 3, per_pass=True, log2_batch=bb)
+            tot = 1 << (bn + bb)
+            batched.append({"n": bn, "log2_batch": bb, "passes": r["passes"], "median_ms": r["median_ms"],
+                            "gflops": 5.0 * tot * bn / (r["median_ms"] * 1e-3) / 1e9,
+                            "gbs": r["passes"] * 16.0 * tot / (r["median_ms"] * 1e-3) / 1e9, "pass_ms": r["pass_ms"]})
+            r["plan"].close()
+            del r
+            torch.cuda.empty_cache()
+
     # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N = 1 only ----
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -422,6 +443,8 @@ def main():
         }
         if sweep:
             line["sweep"] = sweep
+        if batched:
+            line["batched"] = batched
         print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist

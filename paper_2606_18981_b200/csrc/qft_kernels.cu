@@ -266,7 +266,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
     cfg.blockDim = dim3(1u << d.log2_threads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     cfg.attrs = attr;
     cfg.numAttrs = 0;
     if (d.npair > 0) {
@@ -275,6 +275,14 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
         attr[0].val.clusterDim.y = 1;
         attr[0].val.clusterDim.z = 1;
         cfg.numAttrs = 1;
+    }
+    // Programmatic dependent launch: the kernel's prologue (barrier init, phase tables) may overlap the tail
+    // of the previous pass; it executes griddepcontrol.wait before it touches the state.
+    static const bool pdl = []() { const char* e = getenv("QFT_NO_PDL"); return !(e && atoi(e)); }();
+    if (pdl && !pp) {
+        attr[cfg.numAttrs].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[cfg.numAttrs].val.programmaticStreamSerializationAllowed = 1;
+        ++cfg.numAttrs;
     }
     void* args[3] = {(void*)&state, (void*)&map, (void*)&d};
     return cudaLaunchKernelExC(&cfg, (const void*)kern, args);

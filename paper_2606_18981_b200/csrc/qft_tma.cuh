@@ -142,6 +142,8 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     const int win_lo = d.win_lo;
     const uint64_t lbmask = (win_lo > 0) ? ((1ull << win_lo) - 1ull) : 0ull;
 
+    // let the next pass's CTAs be scheduled as soon as SM resources free up (they wait below)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0) {
         mbar_init(mbar, 1);
         fence_proxy_async();
@@ -178,6 +180,9 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         for (int j = 0; j < 5; ++j) c[j] = (int)((base >> t.tma_lo[j]) & ((1ull << t.tma_len[j]) - 1ull));
     };
 
+    // everything above is independent of the state; the previous pass must have completed (and its
+    // writes be visible) before the first load
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     uint32_t unit = blockIdx.x / csz;
     if (unit < nunits && tid == 0) {
         int c[5];

@@ -68,3 +68,34 @@ def test_tma2_matches_generic_kernel_bitwise_layout():
     peak = int(torch.argmax(outs[0].abs()).item())
     assert peak == 12345
     assert abs(abs(outs[0][peak].item()) - 1.0) <= 1e-4
+
+
+def test_plan_reuse_across_streams_and_states():
+    """A plan is immutable and reusable (include/qft.h): the same plan on two streams, two states in
+    flight at once, several executes back to back (programmatic dependent launch between the passes),
+    then exact-k round trip sign=-1 / sign=+1 back to the input."""
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    n = 21
+    xa, xb = qi.gaussian(n, 1), qi.gaussian(n, 2)
+    fwd = qft.Plan(n, n)
+    inv = qft.Plan(n, n, sign=1)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    ta, tb = torch.from_numpy(xa).cuda(), torch.from_numpy(xb).cuda()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        fwd.execute(ta, sa.cuda_stream)
+        fwd.execute(tb, sb.cuda_stream)
+        inv.execute(ta, sa.cuda_stream)
+        inv.execute(tb, sb.cuda_stream)
+    fwd.execute(ta, sa.cuda_stream)
+    torch.cuda.synchronize()
+    ref = oracle.qft(xa)
+    got = ta.cpu().numpy().astype(np.complex128)
+    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 1e-4
+    back = tb.cpu().numpy().astype(np.complex128)
+    assert float(np.linalg.norm(back - xb) / np.linalg.norm(xb)) <= 1e-4
+    fwd.close()
+    inv.close()

@@ -176,3 +176,33 @@ def test_error_codes_on_device():
     with pytest.raises(qft.QftError):
         qft.qft_execute(plan.handle, 0, 0)  # null
     plan.close()
+
+
+def test_aqft_accuracy_vs_cutoff_paper_workload():
+    """The paper's AQFT accuracy experiment (Fig. 6): n = 22, single tone at bin 2, unit
+    norm; infidelity 1 - F against the exact output and top-bin leakage, both falling as k grows.  The
+    GPU path must reproduce the oracle's values, and both follow (4 pi^2 / 3) 4^-(k+2), the closed form
+    the product formula of the AQFT gives for a low-frequency tone."""
+    n, f = 22, 2
+    x = qi.tone(n, f)
+    exact = gpu_qft(x).astype(np.complex128)
+    assert abs(abs(exact[f]) - 1.0) <= 1e-5
+    prev = None
+    for k in (4, 6, 8, 10):
+        got = gpu_qft(x, k).astype(np.complex128)
+        ref = oracle.qft(x, k)
+        assert rel_l2(got, ref) <= TOL_LARGE
+
+        def metrics(out):
+            leak = 1.0 - abs(out[f]) ** 2 / float(np.vdot(out, out).real)
+            fid = abs(np.vdot(exact, out)) ** 2 / float(np.vdot(exact, exact).real * np.vdot(out, out).real)
+            return leak, 1.0 - fid
+
+        (lg, ig), (lo, io) = metrics(got), metrics(ref)
+        pred = (4.0 * math.pi ** 2 / 3.0) * 4.0 ** (-(k + 2))
+        assert abs(lo - pred) <= 0.05 * pred            # the oracle follows the closed form
+        assert abs(lg - lo) <= 0.02 * lo + 2e-6          # the GPU path follows the oracle (fp32 floor ~1e-6)
+        assert abs(ig - io) <= 0.02 * io + 2e-6
+        if prev is not None:
+            assert lg < prev                             # monotone in k (PAPER.md:201)
+        prev = lg

@@ -149,6 +149,25 @@ qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_
  * pairing, kernel).  Writes at most len-1 characters plus a NUL; returns
  * QFT_ERR_INVALID_ARG if the buffer is too small (8 KiB is always enough). */
 qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len);
+/*
+ * The steps either side of the circuit.  All take a device pointer to
+ * float2[2^n_qubits] (16-byte aligned, n_qubits >= 1), accumulate in double precision, return a number
+ * to the host and therefore SYNCHRONISE the stream (qft_rescale only enqueues).
+ *   qft_norm_sq     *norm_sq_out = sum_j |x_j|^2.
+ *   qft_encode    amplitude encoding of PAPER.md:124: *scale_in_out = ||x||_2 and x /= scale_in, in place;
+ *                 QFT_ERR_INVALID_ARG for the zero vector.
+ *   qft_rescale   x *= factor, in place: the decode step of PAPER.md:139 (factor = scale_in for the unitary
+ *                 convention, scale_in * sqrt(N) for the unnormalised DFT).
+ *   qft_fidelity  *fidelity_out = |<a,b>|^2 / (||a||^2 ||b||^2).
+ *   qft_leakage   *leakage_out = 1 - |x[bin]|^2 / ||x||^2: the top-bin leakage of PAPER.md:181.
+ */
+qft_status_t qft_norm_sq(const void* device_state, int n_qubits, double* norm_sq_out, void* stream);
+qft_status_t qft_encode(void* device_state, int n_qubits, double* scale_in_out, void* stream);
+qft_status_t qft_rescale(void* device_state, int n_qubits, double factor, void* stream);
+qft_status_t qft_fidelity(const void* device_a, const void* device_b, int n_qubits, double* fidelity_out, void* stream);
+qft_status_t qft_leakage(const void* device_state, int n_qubits, unsigned long long bin, double* leakage_out,
+                         void* stream);
+
 /* Re-runs the planner's host-side proof: follows every qubit through every
  * pass's address permutation and checks that each gate's target was inside the
  * tile when applied, that tiles are closed under the store permutation, and

@@ -173,3 +173,32 @@ def outputs_at(x, Ks, k: int | None = None, sign: int = -1, norm: int = NORM_UNI
     lib().orc_outputs_at(x.ctypes.data_as(ctypes.c_void_p), is_f32, n, k, sign, norm,
                          Ks.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), Ks.shape[0], _dp(out))
     return out
+
+
+# ---- the steps either side of the circuit, written out from their definitions ----
+
+def norm_sq(x) -> float:
+    """sum_j |x_j|^2 in float64 (the square of scale_in)."""
+    a = np.asarray(x, dtype=np.complex128).ravel()
+    return float(np.sum(a.real * a.real + a.imag * a.imag))
+
+
+def encode(x):
+    """amplitude encoding; returns (x / scale_in, scale_in) with scale_in = ||x||_2."""
+    a = np.asarray(x, dtype=np.complex128).ravel()
+    scale_in = float(np.sqrt(norm_sq(a)))
+    return a / scale_in, scale_in
+
+
+def fidelity(a, b) -> float:
+    """PAPER.md:181: F = |<a, b>|^2 / (||a||^2 ||b||^2)."""
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    inner = np.sum(np.conj(a) * b)
+    return float((inner.real ** 2 + inner.imag ** 2) / (norm_sq(a) * norm_sq(b)))
+
+
+def leakage(out, k0: int) -> float:
+    """top-bin leakage 1 - |out[k0]|^2 / ||out||^2."""
+    o = np.asarray(out, dtype=np.complex128).ravel()
+    return float(1.0 - (o[k0].real ** 2 + o[k0].imag ** 2) / norm_sq(o))

@@ -28,6 +28,7 @@ EXPORTS = [
     "qft_plan_create", "qft_plan_create_batched", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
     "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
+    "qft_norm_sq", "qft_encode", "qft_rescale", "qft_fidelity", "qft_leakage",
 ]
 
 _lib = None
@@ -84,6 +85,14 @@ def load() -> ctypes.CDLL:
     L.qft_plan_self_check.restype = ci
     L.qft_status_string.argtypes = [ci]
     L.qft_status_string.restype = ctypes.c_char_p
+    dp = ctypes.POINTER(ctypes.c_double)
+    L.qft_norm_sq.argtypes = [vp, ci, dp, vp]
+    L.qft_encode.argtypes = [vp, ci, dp, vp]
+    L.qft_rescale.argtypes = [vp, ci, ctypes.c_double, vp]
+    L.qft_fidelity.argtypes = [vp, vp, ci, dp, vp]
+    L.qft_leakage.argtypes = [vp, ci, ctypes.c_ulonglong, dp, vp]
+    for _f in (L.qft_norm_sq, L.qft_encode, L.qft_rescale, L.qft_fidelity, L.qft_leakage):
+        _f.restype = ci
     L.qft_last_cuda_error.argtypes = []
     L.qft_last_cuda_error.restype = ctypes.c_char_p
     _lib = L
@@ -180,6 +189,38 @@ def qft_plan_self_check(plan: int) -> None:
     st = load().qft_plan_self_check(plan)
     if st != QFT_OK:
         raise QftError(st, "qft_plan_self_check")
+
+
+def _dbl_call(name: str, *args) -> float:
+    out = ctypes.c_double()
+    fn = getattr(load(), name)
+    st = fn(*args[:-1], ctypes.byref(out), args[-1])
+    if st != QFT_OK:
+        raise QftError(st, name)
+    return out.value
+
+
+def qft_norm_sq(device_state_ptr: int, n_qubits: int, stream: int = 0) -> float:
+    return _dbl_call("qft_norm_sq", device_state_ptr, n_qubits, stream)
+
+
+def qft_encode(device_state_ptr: int, n_qubits: int, stream: int = 0) -> float:
+    """Divides the state by its L2 norm in place and returns that norm (scale_in)."""
+    return _dbl_call("qft_encode", device_state_ptr, n_qubits, stream)
+
+
+def qft_rescale(device_state_ptr: int, n_qubits: int, factor: float, stream: int = 0) -> None:
+    st = load().qft_rescale(device_state_ptr, n_qubits, float(factor), stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_rescale")
+
+
+def qft_fidelity(device_a_ptr: int, device_b_ptr: int, n_qubits: int, stream: int = 0) -> float:
+    return _dbl_call("qft_fidelity", device_a_ptr, device_b_ptr, n_qubits, stream)
+
+
+def qft_leakage(device_state_ptr: int, n_qubits: int, bin_index: int, stream: int = 0) -> float:
+    return _dbl_call("qft_leakage", device_state_ptr, n_qubits, int(bin_index), stream)
 
 
 class Plan:

@@ -481,3 +481,26 @@ def test_input_recipes():
     assert abs(np.linalg.norm(t.astype(np.complex128)) - 1) < 1e-6
     d = qi.delta(10, 777)
     assert d[777] == 1 and np.count_nonzero(d) == 1
+
+
+def test_metric_definitions_closed_forms():
+    """Pins of oracle.norm_sq / encode / fidelity / leakage to cases with a known value."""
+    rng = np.random.default_rng(11)
+    a = rng.normal(size=64) + 1j * rng.normal(size=64)
+    assert abs(oracle.norm_sq([3 + 4j, 0, 12j]) - 169.0) < 1e-12          # 3-4-5 and 5-12-13
+    e, s = oracle.encode([3 + 4j, 0, 12j])
+    assert abs(s - 13.0) < 1e-12 and abs(oracle.norm_sq(e) - 1.0) < 1e-12
+    assert abs(oracle.fidelity(a, a) - 1.0) < 1e-12
+    assert abs(oracle.fidelity(a, (2 - 3j) * a) - 1.0) < 1e-12            # insensitive to scale and global phase
+    u = np.zeros(8, complex); v = np.zeros(8, complex); u[1] = 1; v[5] = 1j
+    assert oracle.fidelity(u, v) == 0.0                                     # orthogonal states
+    assert abs(oracle.fidelity(u, (u + v) / np.sqrt(2)) - 0.5) < 1e-12
+    assert oracle.leakage(u, 1) == 0.0 and oracle.leakage(u, 2) == 1.0
+    assert abs(oracle.leakage([1, 1, 1, 1], 3) - 0.75) < 1e-12
+    # for a single-tone input the AQFT's infidelity against the exact output equals its top-bin leakage
+    n, f = 8, 2
+    x = qi.tone(n, f)
+    exact = oracle.qft(x)
+    for k in (2, 4):
+        out = oracle.qft(x, k)
+        assert abs((1.0 - oracle.fidelity(exact, out)) - oracle.leakage(out, f)) < 1e-7  # complex64 input rounding

@@ -76,8 +76,12 @@ typedef enum {
  *                     when n > 13) are clamped, not an error.  The result does
  *                     not depend on it, only the number of passes does.
  *   sign              -1: the paper's forward transform; +1: every phase
- *                     conjugated (the inverse DFT when k >= n-1; for k < n-1 it
- *                     is the conjugated AQFT, not the inverse of the forward AQFT).
+ *                     conjugated.  With unitary normalisation this is the exact
+ *                     inverse of the sign = -1 transform with the same k, for every
+ *                     k: the (A)QFT matrix including the swaps is symmetric (the
+ *                     gate list read backwards is the same circuit on the reversed
+ *                     qubit order, reading c12), so its inverse, the
+ *                     conjugate transpose, is its conjugate.
  *   normalisation     see qft_norm_t.
  */
 qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,

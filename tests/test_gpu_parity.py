@@ -206,3 +206,12 @@ def test_aqft_accuracy_vs_cutoff_paper_workload():
         if prev is not None:
             assert lg < prev                             # monotone in k
         prev = lg
+
+
+@pytest.mark.parametrize("n,k", [(12, 2), (18, 3), (22, 5), (24, 0)])
+def test_aqft_round_trip(n, k):
+    """sign = +1 with the same cutoff inverts the forward AQFT (reading c12)."""
+    x = qi.gaussian(n, 9)
+    y = gpu_qft(x, k)
+    z = gpu_qft(y, k, sign=1)
+    assert rel_l2(z, x) <= tol(n)

@@ -504,3 +504,23 @@ def test_metric_definitions_closed_forms():
     for k in (2, 4):
         out = oracle.qft(x, k)
         assert abs((1.0 - oracle.fidelity(exact, out)) - oracle.leakage(out, f)) < 1e-7  # complex64 input rounding
+
+
+def test_aqft_matrix_is_symmetric_so_conjugate_is_inverse():
+    """DESIGN.md reading c12: the (A)QFT matrix including the swaps is symmetric for every cutoff k
+    (H and CR are symmetric, the kept rotations are invariant under q -> n-1-q, the reversed gate list is
+    the same circuit on the reversed qubit order), hence its inverse is its complex conjugate: sign = +1
+    undoes sign = -1 with the same k.  Checked on the oracle's full matrix and by round trips."""
+    for n in (1, 2, 3, 4, 6):
+        N = 1 << n
+        eye = np.eye(N, dtype=np.complex128)
+        for k in range(0, n + 1):
+            A = np.stack([oracle.qft(eye[j], k) for j in range(N)], axis=1)      # columns = images of basis states
+            assert np.abs(A - A.T).max() < 1e-14
+            assert np.abs(A.conj().T @ A - eye).max() < 1e-13                     # unitary (PAPER.md:138)
+            B = np.stack([oracle.qft(eye[j], k, sign=1) for j in range(N)], axis=1)
+            assert np.abs(B - A.conj()).max() < 1e-14
+            assert np.abs(B @ A - eye).max() < 1e-13
+    x = qi.gaussian(10, 3).astype(np.complex128)
+    for k in (0, 1, 3, 5):
+        assert np.linalg.norm(oracle.qft(oracle.qft(x, k), k, sign=1) - x) < 1e-13

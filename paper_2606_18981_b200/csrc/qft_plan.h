@@ -23,8 +23,8 @@
 #define QFT_MAX_STEPS 14
 #define QFT_MAX_RADIX_BITS 5
 // QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, 2 x 32 rows of end bases, one mbarrier, 5 coords
-#define QFT_TMA2_MID_STRIDE 8   // float2 per row (R1 <= 5 used)
-#define QFT_TMA2_END_STRIDE 16  // float2 per row (R1 + R2 <= 10 used)
+#define QFT_TMA2_MID_STRIDE 9   // float2 per row (<= 5 used; odd: rows of different lanes fall into different banks)
+#define QFT_TMA2_END_STRIDE 17  // float2 per row (R1 + R2 <= 10 used; odd for the same reason)
 // QFT_KERNEL_TMA2PP: 1 KB alignment slack + landing (2^14) + exchange (2^13) + mid + 4 end tables + mbarrier etc.
 #define QFT_TMA2PP_SMEM_BYTES (1024 + (8 << 14) + (8 << 13) + (32 * QFT_TMA2_MID_STRIDE + 4 * 32 * QFT_TMA2_END_STRIDE) * 8 + 8 + 48 + 8)
 #define QFT_TMA2_TABLE_BYTES(eb) ((32 * QFT_TMA2_MID_STRIDE + 2 * ((eb) > 5 ? (1 << (eb)) : 32) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)

@@ -166,3 +166,38 @@ def test_config5_n33_tones_exact_and_k16():
         if k == 33:
             g5 = x[torch.as_tensor(fr, device="cuda")].to(torch.complex128).cpu().numpy()
             assert np.max(np.abs(g5 - np.exp(1j * ph) / math.sqrt(5))) < 1e-4
+
+
+def test_max_size_n34_tones_exact():
+    """The largest state the ABI accepts (n = 34: 128 GiB in place on a 180 GB B200): five tones against the
+    closed form on sampled chunks, Parseval, and direct double-precision sums at sampled outputs."""
+    import torch
+
+    import large_checks as lc
+    import paper_2606_18981_b200 as qft
+
+    if _free_gib() < 136:
+        pytest.skip("needs 136 GiB of free device memory")
+    n = 34
+    fr, ph = qi.tone_params(n, 5, 5)
+    x = torch.empty(1 << n, dtype=torch.complex64, device="cuda")
+    qi.multi_tone_device(n, fr, ph, device="cuda", out=x)
+    assert abs(lc.norm2(x) - 1.0) < 1e-5
+    Ks = _sample_indices(n, fr, 35, 8)
+    want = lc.sampled_outputs(x, Ks, n)
+    plan = qft.Plan(n, n)
+    plan.self_check()
+    plan.execute(x)
+    torch.cuda.synchronize()
+    plan.close()
+    assert abs(lc.norm2(x) - 1.0) < 1e-4
+    got = x[torch.as_tensor(Ks, device="cuda")].to(torch.complex128)
+    err = float(torch.linalg.vector_norm(got - want).item() / torch.linalg.vector_norm(want).item())
+    assert err <= TOL_LARGE, err
+    rng = np.random.default_rng(34)
+    near = sorted({int(f) >> 22 for f in fr})
+    chunks = sorted(set(near) | {int(c) for c in rng.integers(0, 1 << (n - 22), size=24)})
+    rel, _ = lc.tones_rel_l2(x, n, n, fr, ph, chunk_bits=22, index_chunks=chunks)
+    assert rel <= TOL_LARGE, rel
+    g5 = x[torch.as_tensor(fr, device="cuda")].to(torch.complex128).cpu().numpy()
+    assert np.max(np.abs(g5 - np.exp(1j * ph) / math.sqrt(5))) < 1e-4

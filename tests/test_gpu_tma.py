@@ -99,3 +99,37 @@ def test_plan_reuse_across_streams_and_states():
     assert float(np.linalg.norm(back - xb) / np.linalg.norm(xb)) <= 1e-4
     fwd.close()
     inv.close()
+
+
+def test_execute_is_cuda_graph_capturable():
+    """qft_execute only enqueues kernels (tensor maps are kernel parameters encoded on the host), so a whole
+    transform can be captured into a CUDA graph and replayed - the launch-bound regime of the paper's sizes."""
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    n = 18
+    x = qi.gaussian(n, 4)
+    plan = qft.Plan(n, n)
+    t = torch.from_numpy(x).cuda()
+    s = torch.cuda.Stream()
+    plan.execute(t, s.cuda_stream)  # warm-up outside the capture
+    torch.cuda.synchronize()
+    t.copy_(torch.from_numpy(x).cuda())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        plan.execute(t, s.cuda_stream)
+    g.replay()
+    torch.cuda.synchronize()
+    ref = oracle.qft(x)
+    got = t.cpu().numpy().astype(np.complex128)
+    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 2e-5
+    # replay on fresh data gives the transform of the fresh data
+    y = qi.gaussian(n, 5)
+    t.copy_(torch.from_numpy(y).cuda())
+    g.replay()
+    torch.cuda.synchronize()
+    ref = oracle.qft(y)
+    got = t.cpu().numpy().astype(np.complex128)
+    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 2e-5
+    plan.close()

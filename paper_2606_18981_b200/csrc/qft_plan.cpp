@@ -26,6 +26,7 @@ struct PassSpec {
     std::vector<int> window;                 // logical qubits, descending; empty = permutation only
     std::vector<int> F;                      // tile address bits
     std::vector<int> Fbase;                  // F before the passive extras were added
+    int extras_above = -1;                   // >= 0: take passive extras from address bits above this one first
     std::vector<std::pair<int, int>> moves;  // in-tile: data on address first goes to address second
     std::vector<std::pair<int, int>> swaps;  // non-tile address pairs (lo, hi) that trade places
 };
@@ -38,6 +39,14 @@ void add_extras(PassSpec& ps, int n, int ftarget) {
     std::set<int> used(ps.F.begin(), ps.F.end());
     std::set<int> sw;
     for (auto& s : ps.swaps) { sw.insert(s.first); sw.insert(s.second); }
+    // natural-order passes: the bits right above the window hold qubits that are already processed, which
+    // contribute no phases (fewer table rows) and extend the window's run (fewer tensor-map dims)
+    if (ps.extras_above >= 0)
+        for (int a = ps.extras_above + 1; a < n && (int)ps.F.size() < ftarget; ++a) {
+            if (used.count(a) || sw.count(a)) continue;
+            ps.F.push_back(a);
+            used.insert(a);
+        }
     for (int a = 0; a < n && (int)ps.F.size() < ftarget; ++a) {
         if (used.count(a) || sw.count(a)) continue;
         ps.F.push_back(a);
@@ -66,6 +75,7 @@ void build_unfolded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out
         for (int a = 0; a < std::min(l, n); ++a) F.insert(a);
         for (int q : ps.window) F.insert(q);
         ps.F.assign(F.begin(), F.end());
+        if (n > fmax) ps.extras_above = t;
         add_extras(ps, n, f);
         t -= sizes[p];
         out->push_back(ps);
@@ -146,7 +156,7 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) 
 
 std::vector<int> step_sizes(int w, bool force2 = false) {
     if (w <= 0) return {};
-    if (force2 && (w == 4 || w == 5)) return split_balanced(w, 2);  // two register groups for the TMA kernel
+    if (force2 && w >= 2 && w <= 5) return split_balanced(w, 2);  // two register groups for the TMA kernel
     const int g = ilog2_ceil_div(w, QFT_MAX_RADIX_BITS);
     return split_balanced(w, g);  // larger groups first
 }
@@ -223,7 +233,8 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     const int r1 = s1.r, r2 = s2.r;
     if (f < 12 || f > 14) QFT_REJECT(2);
     if (!((r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3) ||
-          (r1 == 3 && r2 == 3) || (r1 == 3 && r2 == 2) || (r1 == 2 && r2 == 2)))
+          (r1 == 3 && r2 == 3) || (r1 == 3 && r2 == 2) || (r1 == 2 && r2 == 2) || (r1 == 2 && r2 == 1) ||
+          (r1 == 1 && r2 == 1)))
         QFT_REJECT(3);
     if (pp && r1 + r2 < 7) QFT_REJECT(4);
     if (s1.a != s2.a + r2) QFT_REJECT(5);  // the window is one run of canonical bits
@@ -613,7 +624,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         {
             // the passive extra tile bits are optional: if the full tile does not fit the TMA kernel
             // (too many tensor-map dims, too many low in-tile qubits), try smaller tiles
-            const bool want_tma = !(prm.flags & 5u) && ps.window.size() >= 4;
+            const bool want_tma = !(prm.flags & 5u) && ps.window.size() >= 2;
             bool done = false;
             if (want_tma && !ps.Fbase.empty()) {
                 for (int ft = (int)ps.F.size(); ft >= 12 && ft >= (int)ps.Fbase.size() && !done; --ft) {

@@ -24,5 +24,7 @@ static tma2_kernel_t qft_pick_tma2_kc(int kc) {
         if (r1 == 3 && r2 == 3) return qft_pick_tma2_kc<3, 3, LT>(kc);    \
         if (r1 == 3 && r2 == 2) return qft_pick_tma2_kc<3, 2, LT>(kc);    \
         if (r1 == 2 && r2 == 2) return qft_pick_tma2_kc<2, 2, LT>(kc);    \
+        if (r1 == 2 && r2 == 1) return qft_pick_tma2_kc<2, 1, LT>(kc);    \
+        if (r1 == 1 && r2 == 1) return qft_pick_tma2_kc<1, 1, LT>(kc);    \
         return nullptr;                                                   \
     }

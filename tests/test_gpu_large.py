@@ -20,6 +20,7 @@ TOL_LARGE = 1e-4  # north_star: relative L2 <= 1e-4 up to n = 33
 def _free_gib():
     import torch
 
+    torch.cuda.empty_cache()  # earlier tests' cached blocks count as used otherwise
     free, _ = torch.cuda.mem_get_info()
     return free / 2 ** 30
 

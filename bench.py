@@ -220,6 +220,13 @@ def oracle_sample(n, k, reps=1):
     return est, spent, desc, oracle.max_threads()
 
 
+def workload_text(n, k):
+    """The workload both arms report (config.workload)."""
+    return (f"n={n} {'exact QFT' if k is None else 'AQFT k=%d' % k}: 2^{n} complex64 amplitudes "
+            f"({8 * (1 << n) / 2 ** 30:.3g} GiB) per GPU, in place, forward sign, unitary scaling, "
+            f"natural order in and out")
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -245,8 +252,9 @@ def run_reference(args):
         "impl": "reference", "metric": "dft_equiv_gflops", "value": gf, "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": steps_run, "warmup": warm_run, "ms_per_step": est * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"n={n} {'exact QFT' if args.k is None else 'AQFT k=%d' % args.k}, "
-                               f"2^{n} amplitudes, CPU oracle (gate-by-gate fp64, OpenMP)"},
+        "config": {"workload": workload_text(n, args.k), "n_qubits": n,
+                   "aqft_cutoff_k": n if args.k is None else min(args.k, n),
+                   "implementation": "CPU oracle (gate-by-gate fp64, OpenMP), bounded sample per step"},
         "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": gf, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -428,9 +436,7 @@ def main():
             "metric": "dft_equiv_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": steps,
             "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"n={n} {'exact QFT' if args.k is None else 'AQFT k=%d' % args.k}: "
-                                   f"2^{n} complex64 amplitudes ({8 * N / 2 ** 30:.3g} GiB) per GPU, in place, "
-                                   f"forward sign, unitary scaling, natural order in and out",
+            "config": {"workload": workload_text(n, args.k),
                        "n_qubits": n, "aqft_cutoff_k": desc["k"], "passes": npass, "ideal_passes": math.ceil(n / 13),
                        "tile_bits": desc["tile_bits"], "hub_bits": desc["hub_bits"], "folded_bit_reversal": desc["folded"],
                        "l2": "state larger than L2, no flush needed" if 8 * N > 2 * 126e6 else

@@ -585,7 +585,8 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     }
     // defaults from the B200 sweep (profiles/r01_tile_hub_sweep.md): 128-byte granules (hub 4) as soon as
     // the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit windows pay off
-    int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : 13);
+    // (n = 13: three multi-CTA passes on 2^12 tiles take 17 us, one 8192-amplitude CTA takes 30 us)
+    int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : (n == 13 && prm.batch_bits == 0 ? 12 : 13));
     int l = prm.hub_bits ? prm.hub_bits : (na >= 20 ? 4 : 3);
     if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 5 || l >= fmax) {
         *err = "unsupported tile_bits / hub_bits";

@@ -118,9 +118,10 @@ qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutof
  *                 by the caller, on the device that is current at the time of the
  *                 call.  No other 2^n-sized buffer is allocated.
  *   stream        a cudaStream_t passed as void* (NULL = the legacy default stream).
- * Only enqueues kernels: no host synchronisation.  The plan is immutable and may
- * be used again, also on other streams (not concurrently from several threads on
- * first use, when the small device tables are created).
+ * Only enqueues kernels: no host synchronisation, no device allocation (the tensor
+ * maps of the TMA kernels are encoded on the host and passed as kernel parameters),
+ * capturable into a CUDA graph.  The plan is immutable: it may be used again, on
+ * other streams and from several threads at once.
  * Errors: QFT_ERR_INVALID_ARG (null / misaligned), QFT_ERR_CUDA (launch failed).
  */
 qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
@@ -130,7 +131,8 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
  * pinned): copies 2^n complex64 to a device buffer owned by the plan (allocated
  * on first use, 8 * 2^n bytes), runs qft_execute, copies the result back into
  * `host_state` and waits for it.  This is the end-to-end entry point timed as
- * "e2e" by bench.py.
+ * "e2e" by bench.py.  Not reentrant on one plan (it owns one staging buffer); for a
+ * batched plan the state has 2^(n_qubits + log2_batch) elements.
  */
 qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream);
 

@@ -72,9 +72,12 @@ typedef enum {
  *   max_fused_qubits  >= 1.  Cap on the number of logical qubits whose gates one
  *                     pass applies (the planner's analogue of qsim's
  *                     max_fused_size).  Values above the device
- *                     limit (the tile holds 13 qubits, up to 10 of them processed
- *                     when n > 13) are clamped, not an error.  The result does
- *                     not depend on it, only the number of passes does.
+ *                     limit are clamped, not an error: a transform that fits one
+ *                     shared-memory tile (n <= 13) is one pass; otherwise a tile holds
+ *                     2^14 amplitudes (2^15 with the tensor-memory extension, n >= 26),
+ *                     of which 4 or 5 address bits are the contiguous granule, so a
+ *                     pass processes up to 10 or 11 qubits.  The result does not
+ *                     depend on it, only the number of passes does.
  *   sign              -1: the paper's forward transform; +1: every phase
  *                     conjugated.  With unitary normalisation this is the exact
  *                     inverse of the sign = -1 transform with the same k, for every
@@ -102,12 +105,13 @@ qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_bat
  * qft_plan_create_tuned -- as qft_plan_create, with the layout knobs exposed for
  * benchmarking: tile_bits (log2 amplitudes per tile, 0 = default), hub_bits
  * (log2 amplitudes per contiguous granule, 0 = default), flags (QFT_FLAG_*).
- * QFT_ERR_UNSUPPORTED if the combination cannot be scheduled.
+ * QFT_ERR_UNSUPPORTED if the combination cannot be scheduled (tile_bits outside 2..14, hub_bits outside
+ * 1..6 or >= tile_bits, tile_bits < 2 * hub_bits for a state larger than a tile, an unknown flag).
  */
 #define QFT_FLAG_GENERIC_ONLY 1u  /* use only the generic shared-memory tile kernel */
 #define QFT_FLAG_UNFOLDED 2u      /* natural-order passes + one stand-alone bit-reversal pass */
 #define QFT_FLAG_NO_TMA 4u        /* do not use the TMA-staged pass kernels */
-#define QFT_FLAG_PINGPONG 8u      /* tile_bits = 14 only: two-group ping-pong variant of the TMA kernel (experimental, slower) */
+#define QFT_FLAG_NO_EXT_TILE 16u  /* do not extend 2^14 tiles by one qubit through tensor memory */
 qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                                    qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
 
@@ -120,9 +124,13 @@ qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutof
  *   stream        a cudaStream_t passed as void* (NULL = the legacy default stream).
  * Only enqueues kernels: no host synchronisation, no device allocation (the tensor
  * maps of the TMA kernels are encoded on the host and passed as kernel parameters),
- * capturable into a CUDA graph.  The plan is immutable: it may be used again, on
- * other streams and from several threads at once.
- * Errors: QFT_ERR_INVALID_ARG (null / misaligned), QFT_ERR_CUDA (launch failed).
+ * capturable into a CUDA graph.  The schedule is immutable; the plan also keeps, per
+ * pass and behind a mutex, the tensor maps it has encoded (keyed by state pointer and
+ * device, four entries) and the device its kernel attributes were set on, so a repeated
+ * call on the same buffer makes no driver call besides the launches.  A plan may be used
+ * again, on other streams and from several threads at once.
+ * Errors: QFT_ERR_INVALID_ARG (null / misaligned), QFT_ERR_CUDA (launch failed, or the
+ * device has no tensor memory / TMA: the library is built for sm_100a only).
  */
 qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
 
@@ -131,8 +139,9 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
  * pinned): copies 2^n complex64 to a device buffer owned by the plan (allocated
  * on first use, 8 * 2^n bytes), runs qft_execute, copies the result back into
  * `host_state` and waits for it.  This is the end-to-end entry point timed as
- * "e2e" by bench.py.  Not reentrant on one plan (it owns one staging buffer); for a
- * batched plan the state has 2^(n_qubits + log2_batch) elements.
+ * "e2e" by bench.py.  Calls on one plan are serialised (it owns one staging buffer, on
+ * the device that was current at the first call; QFT_ERR_INVALID_ARG if another device is
+ * current later); for a batched plan the state has 2^(n_qubits + log2_batch) elements.
  */
 qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream);
 
@@ -151,9 +160,14 @@ qft_status_t qft_plan_destroy(qft_plan_t plan);
 int qft_plan_num_passes(qft_plan_t plan);   /* -1 if plan is NULL */
 int qft_plan_num_launches(qft_plan_t plan); /* kernels one qft_execute enqueues; -1 if NULL */
 qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_cr, long long* n_swap);
-/* JSON text describing every pass (window, tile address bits, steps, permutation,
- * pairing, kernel).  Writes at most len-1 characters plus a NUL; returns
- * QFT_ERR_INVALID_ARG if the buffer is too small (8 KiB is always enough). */
+/* JSON text describing every pass: kernel, tile address bits, window, register steps, store permutation,
+ * pairing, and the fused block's gates ("each descriptor records the participating qubits, the
+ * contiguous subrange of original gates folded into the block"): n_h, n_cr and [gate_first, gate_last], indices
+ * into the time-ordered list  H(q_{n-1}), CR_2(q_{n-2} -> q_{n-1}), ..., H(q_0)  (the swaps follow it and belong to
+ * no pass: they are the passes' store permutations).  Writes at most len-1 characters plus a NUL; returns
+ * QFT_ERR_INVALID_ARG if the buffer is smaller than qft_plan_describe_length(plan) (bytes including the NUL;
+ * 0 if plan is NULL). */
+size_t qft_plan_describe_length(qft_plan_t plan);
 qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len);
 /*
  * The steps either side of the circuit.  All take a device pointer to
@@ -166,7 +180,18 @@ qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len);
  *                 convention, scale_in * sqrt(N) for the unnormalised DFT).
  *   qft_fidelity  *fidelity_out = |<a,b>|^2 / (||a||^2 ||b||^2).
  *   qft_leakage   *leakage_out = 1 - |x[bin]|^2 / ||x||^2: the top-bin leakage of PAPER.md:181.
+ *   qft_num_qubits_for   n = max(1, ceil(log2 length)) of PAPER.md:124 ("we choose n = ceil(log2 N) qubits and
+ *                 allocate a 2^n-element state vector"); -1 if length is 0 or exceeds 2^34.
+ *   qft_encode_padded    the whole input-encoding step of PAPER.md:124 for an array of any length <= 2^n_qubits:
+ *                 copies device_x (float2[length], device memory; may be device_state itself) to the front of
+ *                 device_state (float2[2^n_qubits]), zero-fills the rest, then qft_encode.  Note that the
+ *                 transform of the padded state is the 2^n-point DFT of the padded array, not a length-point DFT.
+ * The reductions keep one 32-byte scratch buffer per device (allocated at the first call on that device) and
+ * serialise calls per device; they cannot be captured into a CUDA graph.
  */
+int qft_num_qubits_for(unsigned long long length);
+qft_status_t qft_encode_padded(void* device_state, int n_qubits, const void* device_x, unsigned long long length,
+                               double* scale_in_out, void* stream);
 qft_status_t qft_norm_sq(const void* device_state, int n_qubits, double* norm_sq_out, void* stream);
 qft_status_t qft_encode(void* device_state, int n_qubits, double* scale_in_out, void* stream);
 qft_status_t qft_rescale(void* device_state, int n_qubits, double factor, void* stream);

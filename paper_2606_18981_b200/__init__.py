@@ -21,12 +21,13 @@ LIB_PATH = os.path.join(_HERE, "libqft.so")
 
 QFT_OK, QFT_ERR_INVALID_ARG, QFT_ERR_UNSUPPORTED, QFT_ERR_ALLOC, QFT_ERR_CUDA, QFT_ERR_INTERNAL = range(6)
 QFT_NORM_UNITARY, QFT_NORM_NONE, QFT_NORM_INV_N = 0, 1, 2
-QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_PINGPONG = 1, 2, 4, 8
+QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_NO_EXT_TILE = 1, 2, 4, 16
 QFT_MAX_QUBITS = 34
 
 EXPORTS = [
     "qft_plan_create", "qft_plan_create_batched", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
     "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
+    "qft_plan_describe_length", "qft_num_qubits_for", "qft_encode_padded",
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
     "qft_norm_sq", "qft_encode", "qft_rescale", "qft_fidelity", "qft_leakage",
 ]
@@ -81,6 +82,12 @@ def load() -> ctypes.CDLL:
     L.qft_plan_gate_counts.restype = ci
     L.qft_plan_describe.argtypes = [vp, ctypes.c_char_p, ctypes.c_size_t]
     L.qft_plan_describe.restype = ci
+    L.qft_plan_describe_length.argtypes = [vp]
+    L.qft_plan_describe_length.restype = ctypes.c_size_t
+    L.qft_num_qubits_for.argtypes = [ctypes.c_ulonglong]
+    L.qft_num_qubits_for.restype = ci
+    L.qft_encode_padded.argtypes = [vp, ci, vp, ctypes.c_ulonglong, ctypes.POINTER(ctypes.c_double), vp]
+    L.qft_encode_padded.restype = ci
     L.qft_plan_self_check.argtypes = [vp]
     L.qft_plan_self_check.restype = ci
     L.qft_status_string.argtypes = [ci]
@@ -177,8 +184,12 @@ def qft_plan_gate_counts(plan: int):
     return a.value, b.value, c.value
 
 
+def qft_plan_describe_length(plan: int) -> int:
+    return int(load().qft_plan_describe_length(plan))
+
+
 def qft_plan_describe(plan: int) -> dict:
-    buf = ctypes.create_string_buffer(1 << 16)
+    buf = ctypes.create_string_buffer(qft_plan_describe_length(plan))
     st = load().qft_plan_describe(plan, buf, len(buf))
     if st != QFT_OK:
         raise QftError(st, "qft_plan_describe")
@@ -207,6 +218,19 @@ def qft_norm_sq(device_state_ptr: int, n_qubits: int, stream: int = 0) -> float:
 def qft_encode(device_state_ptr: int, n_qubits: int, stream: int = 0) -> float:
     """Divides the state by its L2 norm in place and returns that norm (scale_in)."""
     return _dbl_call("qft_encode", device_state_ptr, n_qubits, stream)
+
+
+def qft_num_qubits_for(length: int) -> int:
+    return int(load().qft_num_qubits_for(int(length)))
+
+
+def qft_encode_padded(device_state_ptr: int, n_qubits: int, device_x_ptr: int, length: int, stream: int = 0) -> float:
+    """Copies x (length complex64, device) to the front of the 2^n state, zero-fills the rest, normalises; returns scale_in."""
+    out = ctypes.c_double()
+    st = load().qft_encode_padded(device_state_ptr, n_qubits, device_x_ptr, int(length), ctypes.byref(out), stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_encode_padded")
+    return out.value
 
 
 def qft_rescale(device_state_ptr: int, n_qubits: int, factor: float, stream: int = 0) -> None:

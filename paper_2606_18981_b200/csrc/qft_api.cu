@@ -5,14 +5,17 @@
 #include <new>
 #include <string>
 
-#include "../../include/qft.h"
-#include "qft_plan.h"
+#include <memory>
 
-cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream);
+#include "../../include/qft.h"
+#include "qft_launch.h"
 
 struct qft_plan_s {
     QftHostPlan host;
-    void* dev_buf = nullptr;  // only for qft_execute_host
+    std::unique_ptr<QftPassCache[]> cache;  // one per pass: encoded tensor maps, kernel attributes (qft_launch.h)
+    std::mutex host_mu;                     // serialises qft_execute_host on this plan
+    void* dev_buf = nullptr;                // only for qft_execute_host
+    int dev_buf_device = -1;
     size_t dev_bytes = 0;
 };
 
@@ -25,24 +28,15 @@ static qft_status_t cuda_fail(cudaError_t e) {
 
 extern "C" {
 
-qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
-                                   qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags) {
+static qft_status_t create_from(qft_plan_t* out, const QftPlanParams& prm) {
     if (!out) return QFT_ERR_INVALID_ARG;
-    QftPlanParams prm;
-    prm.n = n_qubits;
-    prm.k = aqft_cutoff_k;
-    prm.max_fused = max_fused_qubits;
-    prm.sign = sign;
-    prm.norm = (int)normalisation;
-    prm.tile_bits = tile_bits;
-    prm.hub_bits = hub_bits;
-    prm.flags = flags;
     qft_plan_s* p = new (std::nothrow) qft_plan_s();
     if (!p) return QFT_ERR_ALLOC;
     std::string err;
     int rc;
     try {
         rc = qft_build_plan(prm, &p->host, &err);
+        if (rc == 0) p->cache.reset(new QftPassCache[p->host.passes.size()]);
     } catch (const std::bad_alloc&) {
         delete p;
         return QFT_ERR_ALLOC;
@@ -59,9 +53,22 @@ qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutof
     return QFT_OK;
 }
 
+qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
+                                   qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags) {
+    QftPlanParams prm;
+    prm.n = n_qubits;
+    prm.k = aqft_cutoff_k;
+    prm.max_fused = max_fused_qubits;
+    prm.sign = sign;
+    prm.norm = (int)normalisation;
+    prm.tile_bits = tile_bits;
+    prm.hub_bits = hub_bits;
+    prm.flags = flags;
+    return create_from(out, prm);
+}
+
 qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_batch, int aqft_cutoff_k,
                                      int max_fused_qubits, int sign, qft_norm_t normalisation) {
-    if (!out) return QFT_ERR_INVALID_ARG;
     QftPlanParams prm;
     prm.n = n_qubits;
     prm.batch_bits = log2_batch;
@@ -69,26 +76,7 @@ qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_bat
     prm.max_fused = max_fused_qubits;
     prm.sign = sign;
     prm.norm = (int)normalisation;
-    qft_plan_s* p = new (std::nothrow) qft_plan_s();
-    if (!p) return QFT_ERR_ALLOC;
-    std::string err;
-    int rc;
-    try {
-        rc = qft_build_plan(prm, &p->host, &err);
-    } catch (const std::bad_alloc&) {
-        delete p;
-        return QFT_ERR_ALLOC;
-    } catch (...) {
-        delete p;
-        return QFT_ERR_INTERNAL;
-    }
-    if (rc != 0) {
-        delete p;
-        g_cuda_err = err;
-        return (qft_status_t)rc;
-    }
-    *out = p;
-    return QFT_OK;
+    return create_from(out, prm);
 }
 
 qft_status_t qft_plan_create(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
@@ -100,8 +88,8 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream) {
     if (!plan || !device_state) return QFT_ERR_INVALID_ARG;
     const uintptr_t align = plan->host.prm.n >= 1 ? 16 : 8;
     if (((uintptr_t)device_state) & (align - 1)) return QFT_ERR_INVALID_ARG;
-    for (const QftPassDesc& d : plan->host.passes) {
-        cudaError_t e = qft_launch_pass(d, device_state, (cudaStream_t)stream);
+    for (size_t i = 0; i < plan->host.passes.size(); ++i) {
+        cudaError_t e = qft_launch_pass(plan->host.passes[i], &plan->cache[i], device_state, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(e);
     }
     return QFT_OK;
@@ -111,7 +99,8 @@ qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_stat
     if (!plan || !device_state || pass_index < 0 || pass_index >= (int)plan->host.passes.size())
         return QFT_ERR_INVALID_ARG;
     if (((uintptr_t)device_state) & 15) return QFT_ERR_INVALID_ARG;
-    cudaError_t e = qft_launch_pass(plan->host.passes[pass_index], device_state, (cudaStream_t)stream);
+    cudaError_t e = qft_launch_pass(plan->host.passes[pass_index], &plan->cache[pass_index], device_state,
+                                    (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return QFT_OK;
 }
@@ -120,16 +109,22 @@ qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream) {
     if (!plan || !host_state) return QFT_ERR_INVALID_ARG;
     const size_t bytes = (size_t)8 << (plan->host.prm.n + plan->host.prm.batch_bits);
     cudaStream_t s = (cudaStream_t)stream;
+    std::lock_guard<std::mutex> lock(plan->host_mu);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
     if (!plan->dev_buf) {
-        cudaError_t e = cudaMalloc(&plan->dev_buf, bytes);
+        e = cudaMalloc(&plan->dev_buf, bytes);
         if (e != cudaSuccess) {
             plan->dev_buf = nullptr;
             g_cuda_err = cudaGetErrorString(e);
             return e == cudaErrorMemoryAllocation ? QFT_ERR_ALLOC : QFT_ERR_CUDA;
         }
         plan->dev_bytes = bytes;
+        plan->dev_buf_device = dev;
     }
-    cudaError_t e = cudaMemcpyAsync(plan->dev_buf, host_state, bytes, cudaMemcpyHostToDevice, s);
+    if (plan->dev_buf_device != dev) return QFT_ERR_INVALID_ARG;  // the staging buffer lives on another device
+    e = cudaMemcpyAsync(plan->dev_buf, host_state, bytes, cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(e);
     qft_status_t st = qft_execute(plan, plan->dev_buf, stream);
     if (st != QFT_OK) return st;
@@ -156,6 +151,15 @@ qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_
     *n_cr = plan->host.n_cr;
     *n_swap = plan->host.n_swap;
     return QFT_OK;
+}
+
+size_t qft_plan_describe_length(qft_plan_t plan) {
+    if (!plan) return 0;
+    try {
+        return qft_describe_plan(plan->host).size() + 1;
+    } catch (...) {
+        return 0;
+    }
 }
 
 qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len) {

@@ -13,12 +13,10 @@
 //      cluster barrier (both CTAs of the pair have finished loading by then, so in place is safe).
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include <stdlib.h>
 
 #include "qft_device.cuh"
 #include "qft_fused.cuh"
-#include <cuda.h>
-#include "qft_plan.h"
+#include "qft_launch.h"
 
 namespace qftk {
 
@@ -176,21 +174,16 @@ static pass_kernel_t pick_kernel(const QftPassDesc& d) {
     return (pass_kernel_t)qftk::qft_tile_pass_generic;
 }
 
-bool qft_fused2_supported(int r1, int r2) {
-    return (r1 == 5 && r2 == 5) || (r1 == 5 && r2 == 4) || (r1 == 4 && r2 == 4) || (r1 == 4 && r2 == 3) ||
-           (r1 == 3 && r2 == 3) || (r1 == 3 && r2 == 2) || (r1 == 2 && r2 == 2);
-}
-
 // ---- QFT_KERNEL_TMA2 ---------------------------------------------------------------------------
 typedef void (*tma2_kernel_t)(float2*, const CUtensorMap, const QftPassDesc);
 tma2_kernel_t qft_pick_tma2_lt7(int r1, int r2, int kc);  // qft_tma_lt7.cu
 tma2_kernel_t qft_pick_tma2_lt8(int r1, int r2, int kc);  // qft_tma_lt8.cu
 tma2_kernel_t qft_pick_tma2_lt9(int r1, int r2, int kc);  // qft_tma_lt9.cu
-tma2_kernel_t qft_pick_tma2pp(int r1, int r2, int kc);    // qft_tma_pp.cu
+tma2_kernel_t qft_pick_tma2_xt(int r1, int r2, int kc);   // qft_tma_xt.cu
 
 static tma2_kernel_t pick_tma2(const QftPassDesc& d) {
     const int kc = d.k < 4 ? d.k : 4;
-    if (d.kernel == QFT_KERNEL_TMA2PP) return qft_pick_tma2pp(d.tma.r1, d.tma.r2, kc);
+    if (d.xt) return d.log2_threads == 9 ? qft_pick_tma2_xt(d.tma.r1, d.tma.r2, kc) : nullptr;
     switch (d.log2_threads) {
         case 7: return qft_pick_tma2_lt7(d.tma.r1, d.tma.r2, kc);
         case 8: return qft_pick_tma2_lt8(d.tma.r1, d.tma.r2, kc);
@@ -215,28 +208,51 @@ static encode_tiled_t get_encode_tiled() {
     return fn;
 }
 
-static int sm_count() {
-    static int n = []() {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) return 148;
-        return v;
-    }();
-    return n;
+static int sm_count(int dev) {
+    static int cached[64] = {0};
+    if (dev < 0 || dev >= 64) return 148;
+    if (cached[dev] > 0) return cached[dev];
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) return 148;
+    cached[dev] = v;  // benign race: every writer stores the same value
+    return v;
 }
 
-int g_qft_tma_l2promo = 1;  // CUtensorMapL2promotion: 0 none, 1 64 B, 2 128 B, 3 256 B (tuning knob)
+static cudaError_t launch_plain(const QftPassDesc& d, QftPassCache* cache, int dev, void* state, cudaStream_t stream) {
+    pass_kernel_t kern = pick_kernel(d);
+    const size_t smem = (size_t)8 << d.f;
+    if (smem > 48 * 1024 && cache->attr_dev != dev) {
+        cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             8 << QFT_MAX_TILE_BITS);
+        if (e != cudaSuccess) return e;
+        cache->attr_dev = dev;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1u << d.ntile);
+    cfg.blockDim = dim3(1u << d.log2_threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    cfg.attrs = attr;
+    cfg.numAttrs = 0;
+    if (d.npair > 0) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.numAttrs = 1;
+    }
+    void* args[2] = {(void*)&state, (void*)&d};
+    return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
+}
 
-static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t stream) {
-    tma2_kernel_t kern = pick_tma2(d);
+// The tensor map of a pass: the state seen as a 5-D tensor over address-bit runs (qft_plan.cpp, lower_tma2).
+// The strides are those of the runs, so a later dimension may have a smaller stride than an earlier one and the
+// tile-index dimension overlaps the others; the driver accepts this today.  If it ever refuses, the caller falls
+// back to the generic kernel (same descriptor, no tensor map).
+static bool encode_map(const QftPassDesc& d, void* state, CUtensorMap* map) {
     encode_tiled_t enc = get_encode_tiled();
-    static const int promo_env = []() {
-        const char* e = getenv("QFT_TMA_L2PROMO");
-        return e ? atoi(e) : -1;
-    }();
-    if (promo_env >= 0 && promo_env <= 3) g_qft_tma_l2promo = promo_env;
-    if (!kern || !enc) return cudaErrorNotSupported;
-    CUtensorMap map;
+    if (!enc) return false;
     cuuint64_t gdim[5], gstr[4];
     cuuint32_t box[5], estr[5];
     for (int i = 0; i < 5; ++i) {
@@ -245,20 +261,50 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
         estr[i] = 1;
         if (i > 0) gstr[i - 1] = 8ull << d.tma.tma_lo[i];
     }
-    CUresult r = enc(&map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 5, state, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     d.kernel == QFT_KERNEL_TMA2PP ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
-                     (CUtensorMapL2promotion)g_qft_tma_l2promo,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-    const bool pp = d.kernel == QFT_KERNEL_TMA2PP;
-    const size_t smem = pp ? (size_t)QFT_TMA2PP_SMEM_BYTES : ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb);
-    cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 5, state, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int dev, void* state, cudaStream_t stream) {
+    tma2_kernel_t kern = pick_tma2(d);
+    if (!kern) return cudaErrorNotSupported;
+    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb);
+    CUtensorMap map;
+    {
+        std::lock_guard<std::mutex> lock(cache->mu);
+        const QftPassCache::Entry* hit = nullptr;
+        for (const auto& e : cache->maps)
+            if (e.ptr == state && e.dev == dev) hit = &e;
+        if (hit) {
+            map = hit->map;
+        } else {
+            if (!encode_map(d, state, &map)) {
+                if (d.xt) return cudaErrorNotSupported;
+                // no tensor map: the generic kernel runs the same descriptor (F = Fst for every plain pass)
+                QftPassDesc g = d;
+                g.kernel = QFT_KERNEL_GENERIC;
+                g.log2_threads = 8;
+                static QftPassCache plain;  // attribute bookkeeping of the fallback only
+                std::lock_guard<std::mutex> lock2(plain.mu);
+                return launch_plain(g, &plain, dev, state, stream);
+            }
+            QftPassCache::Entry& e = cache->maps[cache->next];
+            cache->next = (cache->next + 1) % 4;
+            e.ptr = state;
+            e.dev = dev;
+            e.map = map;
+        }
+        if (cache->attr_dev != dev) {
+            cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            cache->attr_dev = dev;
+        }
+    }
     int per_sm = d.f == 13 ? 2 : (d.f == 12 ? 4 : 1);
     while (per_sm > 1 && per_sm * (smem + 1024) > 227 * 1024) --per_sm;
     const unsigned csz = d.npair ? 2u : 1u;
-    unsigned long long ntiles = 1ull << d.ntile;
-    unsigned long long grid = (unsigned long long)sm_count() * per_sm;
+    unsigned long long ntiles = 1ull << (d.ntile - d.xt);
+    unsigned long long grid = (unsigned long long)sm_count(dev) * per_sm;
     if (grid > ntiles) grid = ntiles;
     grid -= grid % csz;
     cudaLaunchConfig_t cfg = {};
@@ -278,41 +324,18 @@ static cudaError_t launch_tma2(const QftPassDesc& d, void* state, cudaStream_t s
     }
     // Programmatic dependent launch: the kernel's prologue (barrier init, phase tables) may overlap the tail
     // of the previous pass; it executes griddepcontrol.wait before it touches the state.
-    static const bool pdl = []() { const char* e = getenv("QFT_NO_PDL"); return !(e && atoi(e)); }();
-    if (pdl && !pp) {
-        attr[cfg.numAttrs].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[cfg.numAttrs].val.programmaticStreamSerializationAllowed = 1;
-        ++cfg.numAttrs;
-    }
+    attr[cfg.numAttrs].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[cfg.numAttrs].val.programmaticStreamSerializationAllowed = 1;
+    ++cfg.numAttrs;
     void* args[3] = {(void*)&state, (void*)&map, (void*)&d};
     return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
 }
 
-cudaError_t qft_launch_pass(const QftPassDesc& d, void* state, cudaStream_t stream) {
-    if (d.kernel == QFT_KERNEL_TMA2 || d.kernel == QFT_KERNEL_TMA2PP) return launch_tma2(d, state, stream);
-    pass_kernel_t kern = pick_kernel(d);
-    const size_t smem = (size_t)8 << d.f;
-    if (smem > 48 * 1024) {
-        // idempotent and cheap; needed once per kernel instantiation
-        cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             8 << QFT_MAX_TILE_BITS);
-        if (e != cudaSuccess) return e;
-    }
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(1u << d.ntile);
-    cfg.blockDim = dim3(1u << d.log2_threads);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    cfg.attrs = attr;
-    cfg.numAttrs = 0;
-    if (d.npair > 0) {
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 2;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.numAttrs = 1;
-    }
-    void* args[2] = {(void*)&state, (void*)&d};
-    return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
+cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* state, cudaStream_t stream) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (d.kernel == QFT_KERNEL_TMA2) return launch_tma2(d, cache, dev, state, stream);
+    std::lock_guard<std::mutex> lock(cache->mu);
+    return launch_plain(d, cache, dev, state, stream);
 }

@@ -1,0 +1,24 @@
+// qft_launch.h -- the launcher's interface to the C ABI (qft_api.cu).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <mutex>
+
+#include "qft_plan.h"
+
+// Per-pass launch state the plan owns: which device the kernel's attributes were set on, and the tensor
+// maps already encoded for this pass (keyed by state pointer and device), so that a repeated qft_execute
+// on the same buffer does no driver call besides the launch itself.
+struct QftPassCache {
+    std::mutex mu;
+    int attr_dev = -1;
+    int next = 0;
+    struct Entry {
+        void* ptr = nullptr;
+        int dev = -1;
+        CUtensorMap map;
+    } maps[4];
+};
+
+cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* state, cudaStream_t stream);

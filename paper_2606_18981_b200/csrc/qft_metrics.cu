@@ -52,20 +52,39 @@ __global__ void __launch_bounds__(256) qft_scale_kernel(float4* __restrict__ a, 
     }
 }
 
-std::mutex g_mu;
-double* g_dev_sums = nullptr;
+// One 32-byte sums buffer per device, allocated at the first call on that device and kept for the life of the
+// process; a call holds its device's lock until the sums are back on the host (the calls synchronise anyway).
+constexpr int kMaxDevices = 64;
+struct DevScratch {
+    std::mutex mu;
+    double* sums = nullptr;
+    int grid = 0;  // 8 CTAs per SM of that device
+};
+DevScratch g_scratch[kMaxDevices];
+
+int grid_for(int dev) {
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+    return sms * 8;
+}
 
 qft_status_t reduce4(const void* a, const void* b, int n, cudaStream_t s, double out[4]) {
     if (!a || n < 1 || n > 34 || (((uintptr_t)a) & 15) || (b && (((uintptr_t)b) & 15))) return QFT_ERR_INVALID_ARG;
-    std::lock_guard<std::mutex> lock(g_mu);
-    if (!g_dev_sums && cudaMalloc(&g_dev_sums, 4 * sizeof(double)) != cudaSuccess) return QFT_ERR_ALLOC;
-    if (cudaMemsetAsync(g_dev_sums, 0, 4 * sizeof(double), s) != cudaSuccess) return QFT_ERR_CUDA;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return QFT_ERR_CUDA;
+    DevScratch& sc = g_scratch[dev];
+    std::lock_guard<std::mutex> lock(sc.mu);
+    if (!sc.sums) {
+        if (cudaMalloc(&sc.sums, 4 * sizeof(double)) != cudaSuccess) { sc.sums = nullptr; return QFT_ERR_ALLOC; }
+        sc.grid = grid_for(dev);
+    }
+    if (cudaMemsetAsync(sc.sums, 0, 4 * sizeof(double), s) != cudaSuccess) return QFT_ERR_CUDA;
     const unsigned long long npairs = (1ull << n) / 2;  // n >= 1: at least one pair
     unsigned long long blocks = (npairs + 255) / 256;
-    if (blocks > 148ull * 8) blocks = 148ull * 8;
-    qft_reduce4<<<(unsigned)blocks, 256, 0, s>>>((const float4*)a, (const float4*)b, npairs, g_dev_sums);
+    if (blocks > (unsigned long long)sc.grid) blocks = sc.grid;
+    qft_reduce4<<<(unsigned)blocks, 256, 0, s>>>((const float4*)a, (const float4*)b, npairs, sc.sums);
     if (cudaGetLastError() != cudaSuccess) return QFT_ERR_CUDA;
-    if (cudaMemcpyAsync(out, g_dev_sums, 4 * sizeof(double), cudaMemcpyDeviceToHost, s) != cudaSuccess) return QFT_ERR_CUDA;
+    if (cudaMemcpyAsync(out, sc.sums, 4 * sizeof(double), cudaMemcpyDeviceToHost, s) != cudaSuccess) return QFT_ERR_CUDA;
     if (cudaStreamSynchronize(s) != cudaSuccess) return QFT_ERR_CUDA;
     return QFT_OK;
 }
@@ -86,7 +105,10 @@ qft_status_t qft_rescale(void* device_state, int n_qubits, double factor, void* 
     if (!device_state || n_qubits < 1 || n_qubits > 34 || (((uintptr_t)device_state) & 15)) return QFT_ERR_INVALID_ARG;
     const unsigned long long npairs = (1ull << n_qubits) / 2;
     unsigned long long blocks = (npairs + 255) / 256;
-    if (blocks > 148ull * 8) blocks = 148ull * 8;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return QFT_ERR_CUDA;
+    const unsigned long long cap = (unsigned long long)grid_for(dev);
+    if (blocks > cap) blocks = cap;
     qft_scale_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>((float4*)device_state, npairs, (float)factor);
     return cudaGetLastError() == cudaSuccess ? QFT_OK : QFT_ERR_CUDA;
 }
@@ -100,6 +122,29 @@ qft_status_t qft_encode(void* device_state, int n_qubits, double* scale_in_out, 
     const double scale_in = sqrt(n2);
     *scale_in_out = scale_in;
     return qft_rescale(device_state, n_qubits, 1.0 / scale_in, stream);
+}
+
+int qft_num_qubits_for(unsigned long long length) {
+    if (length == 0 || length > (1ull << 34)) return -1;
+    int n = 0;
+    while ((1ull << n) < length) ++n;
+    return n < 1 ? 1 : n;
+}
+
+qft_status_t qft_encode_padded(void* device_state, int n_qubits, const void* device_x, unsigned long long length,
+                               double* scale_in_out, void* stream) {
+    if (!device_state || !device_x || !scale_in_out || n_qubits < 1 || n_qubits > 34 || length == 0 ||
+        length > (1ull << n_qubits) || (((uintptr_t)device_state) & 15))
+        return QFT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (device_x != device_state &&
+        cudaMemcpyAsync(device_state, device_x, 8ull * length, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+        return QFT_ERR_CUDA;
+    const unsigned long long total = 1ull << n_qubits;
+    if (length < total &&
+        cudaMemsetAsync((char*)device_state + 8ull * length, 0, 8ull * (total - length), s) != cudaSuccess)
+        return QFT_ERR_CUDA;
+    return qft_encode(device_state, n_qubits, scale_in_out, stream);
 }
 
 qft_status_t qft_fidelity(const void* device_a, const void* device_b, int n_qubits, double* fidelity_out, void* stream) {

@@ -220,15 +220,18 @@ bool solve_swizzle(const int (&L1)[4], const int (&L2)[4], int f, uint8_t (&lowm
 }
 
 // Fills d->tma and sets d->kernel = QFT_KERNEL_TMA2 when the pass fits the kernel's shape.
-// QFT_PLAN_DEBUG=1 in the environment prints why a pass was not given to the TMA kernel
-#define QFT_REJECT(code)                                                                        \
-    do {                                                                                        \
-        if (getenv("QFT_PLAN_DEBUG")) fprintf(stderr, "lower_tma2(pp=%d): reject at #%d (f=%d r=%d+%d)\n", (int)pp, code, d->f, d->steps[0].r, d->steps[1].r); \
-        return;                                                                                 \
+// Compile with -DQFT_PLAN_DEBUG to print why a pass was not given to the TMA kernel.
+#ifdef QFT_PLAN_DEBUG
+#define QFT_REJECT(code)                                                                                              \
+    do {                                                                                                              \
+        fprintf(stderr, "lower_tma2: reject at #%d (f=%d r=%d+%d)\n", code, d->f, d->steps[0].r, d->steps[1].r);      \
+        return;                                                                                                       \
     } while (0)
-void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
+#else
+#define QFT_REJECT(code) return
+#endif
+void lower_tma2(QftPassDesc* d, int n) {
     const int f = d->f;
-    if (pp && f != 14) QFT_REJECT(1);
     const QftStep s1 = d->steps[0], s2 = d->steps[1];
     const int r1 = s1.r, r2 = s2.r;
     if (f < 12 || f > 14) QFT_REJECT(2);
@@ -236,12 +239,11 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
           (r1 == 3 && r2 == 3) || (r1 == 3 && r2 == 2) || (r1 == 2 && r2 == 2) || (r1 == 2 && r2 == 1) ||
           (r1 == 1 && r2 == 1)))
         QFT_REJECT(3);
-    if (pp && r1 + r2 < 7) QFT_REJECT(4);
+    if (d->xt && (f != 14 || r1 + r2 < 8)) QFT_REJECT(4);  // the extended tile is built for 2^14 halves only
     if (s1.a != s2.a + r2) QFT_REJECT(5);  // the window is one run of canonical bits
     const int eb = s2.a;            // canonical bits below the window
-    if (eb > 7 || (pp && eb > 5)) QFT_REJECT(6);
+    if (eb > 7) QFT_REJECT(6);
     if (n - f < 1) QFT_REJECT(7);
-    (void)hub;
     QftTma2Desc t;
     std::memset(&t, 0, sizeof t);
     const int lt = f - 5;
@@ -276,7 +278,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         int b = a + 1;
         if (inF[a]) {
             // dimension 0 may mix classes (it is the hub); the others may not
-            while (b < n && inF[b] && b - a < ((pp && a == 0) ? 4 : 8) && (cls_of(b) == cls_of(a))) ++b;
+            while (b < n && inF[b] && b - a < 8 && (cls_of(b) == cls_of(a))) ++b;
             dims.push_back({a, b - a, b - a, cls_of(a)});
         }
         a = b;
@@ -292,10 +294,10 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     // (only needed when the hub alone does not fill the four lowest landing bits; otherwise keep the
     // natural, address-ascending order)
     if (need_reorder)
-    std::stable_sort(dims.begin() + 1, dims.end(), [](const Dim& x, const Dim& y) {
-        const int kx = x.cls == 2 ? 1 : 0, ky = y.cls == 2 ? 1 : 0;
-        return kx < ky;
-    });
+        std::stable_sort(dims.begin() + 1, dims.end(), [](const Dim& x, const Dim& y) {
+            const int kx = x.cls == 2 ? 1 : 0, ky = y.cls == 2 ? 1 : 0;
+            return kx < ky;
+        });
     while (dims.size() < 5) dims.push_back({n, 0, 0, -1});  // size-1 padding dims
     int nland = 0;
     std::vector<int> land_idx_of_canon(f, -1);
@@ -314,31 +316,15 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     // step 1: register bits = group 1 (+ batch bits: the highest landing bits outside the group);
     // thread bits = the remaining landing bits, ascending, so lanes read consecutive shared memory
     std::vector<int> reg1, thr1, reg2, thr2;
-    int gcan = -1;  // ping-pong: the canonical bit that splits the tile between the two thread groups
-    if (pp) {
-        if (dims[0].box != 4) QFT_REJECT(12);
-        gcan = canon_at_load[t.land_addr[3]];
-        if (in1(gcan) || in2(gcan)) QFT_REJECT(13);
-    }
     for (int b = 0; b < r1; ++b) reg1.push_back(s1.a + b);
     {
         std::vector<int> rest;
         for (int j = 0; j < f; ++j) {
             const int c = canon_at_load[t.land_addr[j]];
-            if (!in1(c) && c != gcan) rest.push_back(c);
+            if (!in1(c)) rest.push_back(c);
         }
         while ((int)reg1.size() < 5) { reg1.push_back(rest.back()); rest.pop_back(); }
         thr1 = rest;
-        if (pp) {
-            // lanes 0-2 = hub bits 0-2, lane 3 = landing row bit 2 (landing index bit 6): with the 128B
-            // swizzle a half-warp then covers all 32 banks; the group bit is the top thread bit
-            const int c6 = canon_at_load[t.land_addr[6]];
-            auto it = std::find(thr1.begin(), thr1.end(), c6);
-            if (it == thr1.end() || (it - thr1.begin()) < 3) QFT_REJECT(14);
-            thr1.erase(it);
-            thr1.insert(thr1.begin() + 3, c6);
-            thr1.push_back(gcan);
-        }
     }
     // step 2: register bits = group 2 (+ batch bits); thread bits = the remaining store-order bits,
     // ascending, so lanes run along the hub and every warp store covers whole granules
@@ -346,45 +332,29 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     {
         std::vector<int> rest;
         for (int j = 0; j < f; ++j)
-            if (!in2(d->st_canon[j]) && d->st_canon[j] != gcan) rest.push_back(d->st_canon[j]);
+            if (!in2(d->st_canon[j])) rest.push_back(d->st_canon[j]);
         while ((int)reg2.size() < 5) { reg2.push_back(rest.back()); rest.pop_back(); }
         thr2 = rest;
-        if (pp) thr2.push_back(gcan);
     }
     if ((int)thr1.size() != lt || (int)thr2.size() != lt) QFT_REJECT(15);
-    if (pp) {
-        for (int j = 0; j < 3; ++j)
-            if (land_idx_of_canon[thr1[j]] != j || st_idx_of_canon[thr2[j]] != j) QFT_REJECT(16);
-        for (int c : reg1) if (c == gcan) QFT_REJECT(17);
-        for (int c : reg2) if (c == gcan) QFT_REJECT(18);
-    } else {
-        for (int j = 0; j < 4; ++j)
-            if (land_idx_of_canon[thr1[j]] != j) QFT_REJECT(19);
-        // store lanes: at least the three lowest hub bits (64-byte segments); a fourth hub bit that
-        // receives a group-2 qubit becomes a register bit (the two half lines leave the same warp a
-        // few instructions apart and merge in L2)
-        const int hubrun0 = dims[0].box;
-        for (int j = 0; j < std::min(hubrun0, 3); ++j)
-            if (st_idx_of_canon[thr2[j]] != j) QFT_REJECT(20);
-    }
-    // exchange layout: canonical index (ping-pong: with the group bit squeezed out) XOR-swizzled
-    auto xpos = [&](int c) { return (gcan >= 0 && c > gcan) ? c - 1 : c; };
+    for (int j = 0; j < 4; ++j)
+        if (land_idx_of_canon[thr1[j]] != j) QFT_REJECT(19);
+    // store lanes: at least the three lowest hub bits (64-byte segments); a fourth hub bit that
+    // receives a group-2 qubit becomes a register bit (the two half lines leave the same warp a
+    // few instructions apart and merge in L2)
+    const int hubrun0 = dims[0].box;
+    for (int j = 0; j < std::min(hubrun0, 3); ++j)
+        if (st_idx_of_canon[thr2[j]] != j || d->Fst[j] != j) QFT_REJECT(20);
+    // exchange layout: canonical index XOR-swizzled
     int L1[4], L2[4];
-    for (int j = 0; j < 4; ++j) { L1[j] = xpos(thr1[j]); L2[j] = xpos(thr2[j]); }
+    for (int j = 0; j < 4; ++j) { L1[j] = thr1[j]; L2[j] = thr2[j]; }
     uint8_t lowmask[16];
     if (!solve_swizzle(L1, L2, f, lowmask)) QFT_REJECT(21);
     auto midcol = [&](int c) -> uint32_t {
-        if (c == gcan) return 0u;
-        const int p = xpos(c);
-        const uint32_t slot = (p < 4) ? (1u << p) : ((1u << p) ^ lowmask[p]);
+        const uint32_t slot = (c < 4) ? (1u << c) : ((1u << c) ^ lowmask[c]);
         return slot << 3;
     };
-    auto landcol = [&](int c) -> uint32_t {
-        const int j = land_idx_of_canon[c];
-        uint32_t col = 8u << j;
-        if (pp && j >= 4 && j <= 6) col ^= 16u << (j - 4);  // TMA 128B swizzle: byte bits 4-6 ^= bits 7-9
-        return col;
-    };
+    auto landcol = [&](int c) -> uint32_t { return 8u << land_idx_of_canon[c]; };
     auto key1 = [&](int c) -> uint16_t {
         if (in2(c)) return (uint16_t)(1u << (c - s2.a));
         if (c < eb) return (uint16_t)(1u << (8 + c));
@@ -401,7 +371,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         t.s1_tid_key[j] = key1(thr1[j]);
         t.s2_tid_mid[j] = midcol(thr2[j]);
         t.s2_tid_key[j] = key2(thr2[j]);
-        t.s2_tid_addr[j] = d->F[st_idx_of_canon[thr2[j]]];
+        t.s2_tid_addr[j] = d->Fst[st_idx_of_canon[thr2[j]]];
     }
     for (int b = 0; b < 5; ++b) {
         t.s1_reg_ld[b] = landcol(reg1[b]);
@@ -409,7 +379,7 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
         t.s1_reg_key[b] = key1(reg1[b]);
         t.s2_reg_mid[b] = midcol(reg2[b]);
         t.s2_reg_key[b] = key2(reg2[b]);
-        t.s2_reg_addr[b] = d->F[st_idx_of_canon[reg2[b]]];
+        t.s2_reg_addr[b] = d->Fst[st_idx_of_canon[reg2[b]]];
     }
     t.eb = (int8_t)eb;
     for (int c = 0; c < eb; ++c) t.e_log[c] = d->log_canon[c];
@@ -417,77 +387,98 @@ void lower_tma2(QftPassDesc* d, int n, int hub, bool pp) {
     t.t2_lo = (int8_t)(s2.t_hi - r2 + 1);
     t.r1 = (int8_t)r1;
     t.r2 = (int8_t)r2;
-    t.pp = pp ? 1 : 0;
     d->tma = t;
-    d->kernel = pp ? QFT_KERNEL_TMA2PP : QFT_KERNEL_TMA2;
+    d->kernel = QFT_KERNEL_TMA2;
     d->log2_threads = lt;
 }
 
 #undef QFT_REJECT
 // Turn a PassSpec into the kernel descriptor given the current layout; updates qubit_at.
-bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma, bool allow_pp,
-                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err, bool force2 = false) {
+// xt: ps.F is the tile of a tensor-memory extended pass (qft_plan.h): the window's lowest qubit g is taken
+// out of the register steps, its address bit becomes the half-tile index bit, and the descriptor describes
+// one half; the pass must then lower to the TMA kernel (no other kernel knows about the extension).
+bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma,
+                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err, bool force2 = false, bool xt = false) {
     std::memset(d, 0, sizeof(*d));
-    const int f = (int)ps.F.size();
-    if (f > QFT_MAX_TILE_BITS || n - f > QFT_MAX_TILEIDX_BITS) { *err = "tile too large"; return false; }
-    d->n = n; d->f = f; d->ntile = n - f; d->k = k; d->conj = conj; d->scale = 1.0f; d->do_scale = 0;
-    d->kernel = QFT_KERNEL_GENERIC;
-    int lt = f - 2;
-    if (lt < 5) lt = 5;
-    if (lt > 8) lt = 8;
-    d->log2_threads = lt;
-    std::vector<int> inF(n, 0);
-    for (int a : ps.F) inF[a] = 1;
-    // canonical order: in-tile qubits ascending by logical id
-    std::vector<int> qs;
-    for (int a : ps.F) qs.push_back(qubit_at[a]);
-    std::sort(qs.begin(), qs.end());
-    std::vector<int> canon_of_q(n, -1);
-    for (int c = 0; c < f; ++c) { canon_of_q[qs[c]] = c; d->log_canon[c] = (int8_t)qs[c]; }
     std::vector<int> dest(n);
     for (int a = 0; a < n; ++a) dest[a] = a;
+    std::vector<int> inFull(n, 0);
+    for (int a : ps.F) inFull[a] = 1;
     for (auto& m : ps.moves) {
-        if (!inF[m.first] || !inF[m.second]) { *err = "move leaves the tile"; return false; }
+        if (!inFull[m.first] || !inFull[m.second]) { *err = "move leaves the tile"; return false; }
         dest[m.first] = m.second;
-    }
-    for (int j = 0; j < f; ++j) {
-        d->F[j] = (int8_t)ps.F[j];
-        d->ld_canon[j] = (int8_t)canon_of_q[qubit_at[ps.F[j]]];
     }
     std::vector<int> src_of(n, -1);
     for (int a : ps.F) {
         if (src_of[dest[a]] != -1) { *err = "in-tile moves are not a permutation"; return false; }
         src_of[dest[a]] = a;
     }
-    for (int j = 0; j < f; ++j) {
-        if (src_of[ps.F[j]] < 0) { *err = "in-tile moves are not a permutation"; return false; }
-        d->st_canon[j] = (int8_t)canon_of_q[qubit_at[src_of[ps.F[j]]]];
+    for (int a : ps.F)
+        if (src_of[a] < 0) { *err = "in-tile moves are not a permutation"; return false; }
+    // load-side and store-side tile bits
+    std::vector<int> Fld(ps.F), Fst(ps.F);
+    int g = -1, a_g = -1, b_g = -1;
+    if (xt) {
+        if (ps.window.size() < 3) { *err = "extended tile: window too small"; return false; }
+        g = ps.window.back();
+        for (int a : ps.F)
+            if (qubit_at[a] == g) a_g = a;
+        if (a_g < 0) { *err = "extended tile: qubit outside the tile"; return false; }
+        b_g = dest[a_g];
+        if (a_g < hub || b_g < hub) { *err = "extended tile: half-tile bit inside the hub"; return false; }
+        Fld.erase(std::find(Fld.begin(), Fld.end(), a_g));
+        Fst.erase(std::find(Fst.begin(), Fst.end(), b_g));
     }
-    // tile-index bits: swapped pairs first (lo side, then hi side), then the rest ascending
+    const int f = (int)Fld.size();
+    if (f > QFT_MAX_TILE_BITS || n - f > QFT_MAX_TILEIDX_BITS) { *err = "tile too large"; return false; }
+    d->n = n; d->f = f; d->ntile = n - f; d->k = k; d->conj = conj; d->scale = 1.0f; d->do_scale = 0;
+    d->kernel = QFT_KERNEL_GENERIC;
+    d->xt = xt ? 1 : 0;
+    d->xt_q = (int8_t)g; d->xt_ld_addr = (int8_t)a_g; d->xt_st_addr = (int8_t)b_g;
+    int lt = f - 2;
+    if (lt < 5) lt = 5;
+    if (lt > 8) lt = 8;
+    d->log2_threads = lt;
+    // canonical order: the half-tile's qubits ascending by logical id
+    std::vector<int> qs;
+    for (int a : Fld) qs.push_back(qubit_at[a]);
+    std::sort(qs.begin(), qs.end());
+    std::vector<int> canon_of_q(n, -1);
+    for (int c = 0; c < f; ++c) { canon_of_q[qs[c]] = c; d->log_canon[c] = (int8_t)qs[c]; }
+    for (int j = 0; j < f; ++j) {
+        d->F[j] = (int8_t)Fld[j];
+        d->Fst[j] = (int8_t)Fst[j];
+        d->ld_canon[j] = (int8_t)canon_of_q[qubit_at[Fld[j]]];
+        d->st_canon[j] = (int8_t)canon_of_q[qubit_at[src_of[Fst[j]]]];
+    }
+    // tile-index bits: swapped pairs first (lo side, then hi side), then the rest ascending, then the
+    // half-tile bit of an extended pass
     const int p = (int)ps.swaps.size();
     d->npair = p;
     std::vector<int> taken(n, 0);
     for (int i = 0; i < p; ++i) {
         const int a = ps.swaps[i].first, b = ps.swaps[i].second;
-        if (inF[a] || inF[b] || taken[a] || taken[b] || a == b) { *err = "bad swap"; return false; }
+        if (inFull[a] || inFull[b] || taken[a] || taken[b] || a == b) { *err = "bad swap"; return false; }
         taken[a] = taken[b] = 1;
         d->tile_addr[i] = (int8_t)a;
         d->tile_addr[p + i] = (int8_t)b;
     }
     int ti = 2 * p;
     for (int a = 0; a < n; ++a)
-        if (!inF[a] && !taken[a]) d->tile_addr[ti++] = (int8_t)a;
+        if (!inFull[a] && !taken[a]) d->tile_addr[ti++] = (int8_t)a;
+    if (xt) d->tile_addr[ti++] = (int8_t)a_g;
     if (ti != n - f) { *err = "tile index bits do not add up"; return false; }
     for (int i = 0; i < n - f; ++i) d->log_tile[i] = (int8_t)qubit_at[d->tile_addr[i]];
     // steps
     d->win_lo = -1;
     d->nsteps = 0;
     if (!ps.window.empty()) {
-        const int w = (int)ps.window.size();
-        for (int i = 0; i < w; ++i) {
+        const int wfull = (int)ps.window.size();
+        for (int i = 0; i < wfull; ++i)
             if (ps.window[i] != ps.window[0] - i) { *err = "window not contiguous"; return false; }
+        const int w = xt ? wfull - 1 : wfull;
+        for (int i = 0; i < w; ++i)
             if (canon_of_q[ps.window[i]] < 0) { *err = "window qubit outside the tile"; return false; }
-        }
         d->win_lo = ps.window[w - 1];
         int t = ps.window[0];
         for (int r : step_sizes(w, force2)) {
@@ -501,7 +492,7 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
     }
     // fused two-step kernel: eligible when the hub's qubits are not in the register group of the
     // step that touches HBM (so that the lanes of a warp can walk whole granules)
-    if (d->nsteps == 2 && allow_fused) {
+    if (d->nsteps == 2 && allow_fused && !xt) {
         const QftStep s1 = d->steps[0], s2 = d->steps[1];
         auto in_group = [](const QftStep& s, int c) { return c >= s.a && c < s.a + s.r; };
         const int l = std::min(hub, f);
@@ -559,8 +550,8 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
             fix(d->t2_canon, std::min(4, f - s2.r));
         }
     }
-    if (d->nsteps == 2 && allow_tma && allow_pp) lower_tma2(d, n, hub, true);
-    if (d->nsteps == 2 && allow_tma && d->kernel != QFT_KERNEL_TMA2PP) lower_tma2(d, n, hub, false);
+    if (d->nsteps == 2 && allow_tma) lower_tma2(d, n);
+    if (xt && d->kernel != QFT_KERNEL_TMA2) { *err = "extended tile: pass does not fit the TMA kernel"; return false; }
     // apply the permutation to the tracking
     std::vector<int> nq(qubit_at);
     for (int a : ps.F) nq[dest[a]] = qubit_at[a];
@@ -570,6 +561,71 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
 }
 
 }  // namespace
+
+// Lower every pass spec; false if a pass could not be lowered (err says which and why).
+static bool lower_all(const QftPlanParams& prm, std::vector<PassSpec>& specs, int na, int k_eff, int l, int fsmem,
+                      QftHostPlan* out, std::string* err) {
+    std::vector<int> qubit_at(na);
+    for (int a = 0; a < na; ++a) qubit_at[a] = a;
+    const int conj = prm.sign == 1 ? 1 : 0;
+    const bool allow_fused = !(prm.flags & 1u);
+    const bool allow_tma = !(prm.flags & 5u);
+    int wmaxseen = 0;
+    for (auto& ps : specs) {
+        QftPassDesc d;
+        // the passive extra tile bits are optional: if the full tile does not fit the TMA kernel
+        // (too many tensor-map dims, too many low in-tile qubits), try smaller tiles
+        const bool want_tma = allow_tma && ps.window.size() >= 2;
+        const int fbase = (int)(ps.Fbase.empty() ? ps.F.size() : ps.Fbase.size());
+        bool done = false;
+        if (want_tma && !ps.Fbase.empty() && fbase <= fsmem) {
+            for (int ft = std::min((int)ps.F.size(), fsmem); ft >= 12 && ft >= fbase && !done; --ft) {
+                PassSpec trial = ps;
+                add_extras(trial, na, ft);
+                if ((int)trial.F.size() != ft) continue;
+                std::vector<int> qa = qubit_at;
+                QftPassDesc dt;
+                std::string e2;
+                if (lower_pass(trial, na, k_eff, conj, l, allow_fused, true, qa, &dt, &e2, true) &&
+                    dt.kernel == QFT_KERNEL_TMA2) {
+                    d = dt;
+                    qubit_at = qa;
+                    done = true;
+                }
+            }
+        }
+        if (!done && fbase > fsmem) {
+            // the window and the hub need one bit more than a shared-memory tile holds: tensor-memory extension
+            PassSpec trial = ps;
+            add_extras(trial, na, fsmem + 1);
+            std::vector<int> qa = qubit_at;
+            QftPassDesc dt;
+            if ((int)trial.F.size() != fsmem + 1 || !want_tma ||
+                !lower_pass(trial, na, k_eff, conj, l, false, true, qa, &dt, err, true, true))
+                return false;
+            d = dt;
+            qubit_at = qa;
+            done = true;
+        }
+        if (!done && (int)ps.F.size() > fsmem) add_extras(ps, na, fsmem);  // the other kernels: shared-memory tiles
+        if (!done && allow_fused && (ps.window.size() == 4 || ps.window.size() == 5)) {
+            // a 4- or 5-qubit window as two register groups, so that the fused kernel can take it
+            std::vector<int> qa = qubit_at;
+            QftPassDesc dt;
+            std::string e2;
+            if (lower_pass(ps, na, k_eff, conj, l, true, false, qa, &dt, &e2, true) && dt.kernel == QFT_KERNEL_FUSED2) {
+                d = dt;
+                qubit_at = qa;
+                done = true;
+            }
+        }
+        if (!done && !lower_pass(ps, na, k_eff, conj, l, allow_fused, allow_tma, qubit_at, &d, err)) return false;
+        wmaxseen = std::max(wmaxseen, (int)ps.window.size());
+        out->passes.push_back(d);
+    }
+    out->window = wmaxseen;
+    return true;
+}
 
 int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err) {
     const int n = prm.n;                  // qubits of one transform
@@ -583,88 +639,58 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         *err = "invalid argument";
         return 1;
     }
-    // defaults from the B200 sweep (profiles/r01_tile_hub_sweep.md): 128-byte granules (hub 4) as soon as
-    // the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit windows pay off
-    // (n = 13: three multi-CTA passes on 2^12 tiles take 17 us, one 8192-amplitude CTA takes 30 us)
+    if (prm.flags & ~(1u | 2u | 4u | 16u)) { *err = "unknown flag"; return 2; }
+    // defaults from the B200 sweeps (profiles/r01_tile_hub_sweep.md, profiles/r02_tile_hub_sweep.md): 128-byte
+    // granules (hub 4) as soon as the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit
+    // windows pay off (n = 13: three multi-CTA passes on 2^12 tiles take 17 us, one 8192-amplitude CTA takes 30 us)
     int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : (n == 13 && prm.batch_bits == 0 ? 12 : 13));
     int l = prm.hub_bits ? prm.hub_bits : (na >= 20 ? 4 : 3);
-    if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 5 || l >= fmax) {
+    if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 6 || l >= fmax) {
         *err = "unsupported tile_bits / hub_bits";
         return 2;
     }
     if (na - std::min(fmax, na) > 30) { *err = "tile_bits too small for this n"; return 2; }
+    // every tile must contain the hub next to its window (and the stand-alone reversal tile holds the hub twice)
+    if (na > fmax && fmax < 2 * l) { *err = "tile_bits < 2 * hub_bits cannot be scheduled"; return 2; }
     out->prm = prm;
     out->k_eff = std::min(prm.k, n);
     out->tile_bits = fmax;
     out->hub_bits = l;
-    out->passes.clear();
     // gate counters before fusion
     out->n_h = n;
     out->n_cr = 0;
     for (int d = 1; d <= std::min(out->k_eff, n - 1); ++d) out->n_cr += n - d;
     out->n_swap = n / 2;
 
-    std::vector<PassSpec> specs;
-    out->folded = false;
-    if (!(prm.flags & 2u)) out->folded = build_folded(n, prm.max_fused, fmax, l, &specs);
-    if (!out->folded) {
-        specs.clear();
-        // batched transforms that fit one tile: two two-step passes (TMA kernel) beat one three-step pass
-        const int wcap = (prm.batch_bits > 0 && n > 10 && n <= fmax) ? std::min(prm.max_fused, (n + 1) / 2) : prm.max_fused;
-        build_unfolded(n, wcap, fmax, l, &specs);
-    }
-    // batched plans: the batch index occupies address bits [n, na); they hold no qubit (ids >= n stand for
-    // "never processed"), never move, and serve as tile-index bits or passive in-tile bits
-    std::vector<int> qubit_at(na);
-    for (int a = 0; a < na; ++a) qubit_at[a] = a;
-    if (na > n)
-        for (auto& ps : specs) add_extras(ps, na, std::min(fmax, na));
-    int wmaxseen = 0;
-    for (auto& ps : specs) {
-        QftPassDesc d;
-        {
-            // the passive extra tile bits are optional: if the full tile does not fit the TMA kernel
-            // (too many tensor-map dims, too many low in-tile qubits), try smaller tiles
-            const bool want_tma = !(prm.flags & 5u) && ps.window.size() >= 2;
-            bool done = false;
-            if (want_tma && !ps.Fbase.empty()) {
-                for (int ft = (int)ps.F.size(); ft >= 12 && ft >= (int)ps.Fbase.size() && !done; --ft) {
-                    PassSpec trial = ps;
-                    add_extras(trial, na, ft);
-                    if ((int)trial.F.size() != ft) continue;
-                    std::vector<int> qa = qubit_at;
-                    QftPassDesc dt;
-                    std::string e2;
-                    if (lower_pass(trial, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), true,
-                                   (prm.flags & 8u) != 0, qa, &dt, &e2, true) &&
-                        (dt.kernel == QFT_KERNEL_TMA2 || dt.kernel == QFT_KERNEL_TMA2PP)) {
-                        d = dt;
-                        qubit_at = qa;
-                        done = true;
-                    }
-                }
-            }
-            if (!done && !(prm.flags & 1u) && (ps.window.size() == 4 || ps.window.size() == 5)) {
-                // a 4- or 5-qubit window as two register groups, so that the fused kernel can take it
-                std::vector<int> qa = qubit_at;
-                QftPassDesc dt;
-                std::string e2;
-                if (lower_pass(ps, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, true, false, false, qa, &dt, &e2, true) &&
-                    dt.kernel == QFT_KERNEL_FUSED2) {
-                    d = dt;
-                    qubit_at = qa;
-                    done = true;
-                }
-            }
-            if (!done &&
-                !lower_pass(ps, na, out->k_eff, prm.sign == 1 ? 1 : 0, l, !(prm.flags & 1u), !(prm.flags & 5u),
-                            (prm.flags & 8u) != 0, qubit_at, &d, err))
-                return 5;
+    // tensor-memory extended tiles (one more window qubit per pass than the shared-memory tile holds): only for
+    // 2^14 tiles, single transforms, TMA kernels allowed; tried first, dropped if any pass cannot be lowered
+    const bool ext_ok = fmax == 14 && prm.batch_bits == 0 && !(prm.flags & (1u | 2u | 4u | 16u)) && n > fmax + 1;
+    for (int attempt = ext_ok ? 0 : 1; attempt < 2; ++attempt) {
+        const int fplan = attempt == 0 ? fmax + 1 : fmax;  // tile bits the schedule may use
+        std::vector<PassSpec> specs;
+        out->passes.clear();
+        out->ext_tile = attempt == 0;
+        out->folded = false;
+        if (!(prm.flags & 2u)) out->folded = build_folded(n, prm.max_fused, fplan, l, &specs);
+        if (!out->folded) {
+            if (attempt == 0) continue;  // the extension only exists for folded schedules
+            specs.clear();
+            // batched transforms that fit one tile: two two-step passes (TMA kernel) beat one three-step pass
+            const int wcap = (prm.batch_bits > 0 && n > 10 && n <= fmax) ? std::min(prm.max_fused, (n + 1) / 2) : prm.max_fused;
+            build_unfolded(n, wcap, fmax, l, &specs);
         }
-        wmaxseen = std::max(wmaxseen, (int)ps.window.size());
-        out->passes.push_back(d);
+        // batched plans: the batch index occupies address bits [n, na); they hold no qubit (ids >= n stand for
+        // "never processed"), never move, and serve as tile-index bits or passive in-tile bits
+        if (na > n)
+            for (auto& ps : specs) add_extras(ps, na, std::min(fmax, na));
+        std::string e2;
+        if (lower_all(prm, specs, na, out->k_eff, l, fmax, out, &e2)) {
+            out->ext_tile = false;
+            for (const QftPassDesc& d : out->passes) out->ext_tile = out->ext_tile || d.xt;
+            break;
+        }
+        if (attempt == 1) { *err = e2; return 5; }
     }
-    out->window = wmaxseen;
     // normalisation: every H contributes 1/sqrt 2; applied once, in the last pass
     double sc = std::pow(2.0, -0.5 * n);
     if (prm.norm == 1) sc = 1.0;
@@ -697,15 +723,34 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
             return 5;
         };
         if (d.n != n || d.f + d.ntile != n || d.f < 1 || d.f > QFT_MAX_TILE_BITS) return fail("sizes");
-        std::vector<int> inF(n, 0);
+        if (d.xt != 0 && d.xt != 1) return fail("xt");
+        if (d.xt && d.kernel != QFT_KERNEL_TMA2) return fail("extended tile without the TMA kernel");
+        std::vector<int> inF(n, 0), inFst(n, 0);
         for (int j = 0; j < d.f; ++j) {
             if (d.F[j] < 0 || d.F[j] >= n || inF[d.F[j]]) return fail("F not a set of address bits");
             if (j && d.F[j] <= d.F[j - 1]) return fail("F not ascending");
             inF[d.F[j]] = 1;
+            if (d.Fst[j] < 0 || d.Fst[j] >= n || inFst[d.Fst[j]]) return fail("Fst not a set of address bits");
+            if (j && d.Fst[j] <= d.Fst[j - 1]) return fail("Fst not ascending");
+            inFst[d.Fst[j]] = 1;
         }
+        // the tile a CTA owns: load side F (+ the half-tile bit), store side Fst (+ the butterfly's bit);
+        // in place is safe only if the two are the same set of addresses
+        std::vector<int> inTile(inF);
+        if (d.xt) {
+            const int ag = d.xt_ld_addr, bg = d.xt_st_addr;
+            if (ag < 0 || ag >= n || inF[ag] || bg < 0 || bg >= n || inFst[bg]) return fail("extended tile: half-tile bits");
+            inTile[ag] = 1;
+            inFst[bg] = 1;
+            if (d.ntile < 1 || d.tile_addr[d.ntile - 1] != ag) return fail("extended tile: half-tile bit is not the last tile-index bit");
+            if (2 * d.npair > d.ntile - 1) return fail("extended tile: half-tile bit inside a pair");
+            if (qubit_at[ag] != d.xt_q || d.xt_q != d.win_lo - 1) return fail("extended tile: qubit");
+        }
+        for (int a = 0; a < n; ++a)
+            if (inTile[a] != inFst[a]) return fail("store tile differs from load tile (not in place)");
         const int l = std::min(plan.hub_bits, n);
         for (int j = 0; j < std::min(l, d.f); ++j)
-            if (d.F[j] != j) return fail("hub not in tile");
+            if (d.F[j] != j || d.Fst[j] != j) return fail("hub not in tile");
         // canonical map consistent with the tracked layout
         std::vector<int> seen(d.f, 0);
         for (int j = 0; j < d.f; ++j) {
@@ -742,9 +787,13 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 --next_qubit;
             }
         }
-        if (d.kernel == QFT_KERNEL_TMA2 || d.kernel == QFT_KERNEL_TMA2PP) {
-            const bool pp = d.kernel == QFT_KERNEL_TMA2PP;
-            if (pp != (d.tma.pp != 0) || (pp && d.f != 14)) return fail("tma2pp: flag");
+        if (d.nsteps > 0 && d.win_lo != next_qubit + 1) return fail("win_lo");
+        if (d.xt) {
+            // the butterfly between the halves comes after every register step of the pass
+            if (d.xt_q != next_qubit) return fail("extended tile: gates out of circuit order");
+            --next_qubit;
+        }
+        if (d.kernel == QFT_KERNEL_TMA2) {
             // replay the kernel's index maps: every (thread, register) of both steps
             const QftTma2Desc& t = d.tma;
             const int f = d.f, lt = f - 5, nt = 1 << lt;
@@ -763,21 +812,20 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     }
                 if (nl != f) return fail("tma2: landing bits");
             }
-            // canonical index of (tid, B) in each step, recovered from the load / store columns
+            // canonical index of (tid, B) in step 1, recovered from the load columns
             auto canon1 = [&](int tid, int B) {
                 uint32_t off = 0;
                 for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) off ^= t.s1_tid_ld[j];
                 for (int b = 0; b < 5; ++b) if ((B >> b) & 1) off ^= t.s1_reg_ld[b];
-                if (pp) off ^= ((off >> 7) & 7u) << 4;  // undo TMA's 128B swizzle
                 const uint32_t idx = off >> 3;  // landing index
                 uint32_t c = 0;
                 for (int j = 0; j < f; ++j) if ((idx >> j) & 1u) c |= 1u << canon_at_load[t.land_addr[j]];
                 return std::make_pair(idx, c);
             };
-            const int ngrp = pp ? 2 : 1;
-            const uint32_t xslots = pp ? (1u << (f - 1)) : (1u << f);
-            std::vector<int> mid_canon((size_t)ngrp << f, -1);
+            const uint32_t xslots = 1u << f;
+            std::vector<int> mid_canon((size_t)1 << f, -1);
             std::vector<char> seen_ld((size_t)1 << f, 0);
+            for (int b = 0; b < s1.r; ++b) if (t.s1_reg_key[b]) return fail("tma2: group bit in key");
             for (int tid = 0; tid < nt; ++tid) {
                 uint32_t key = 0, offm_t = 0;
                 for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) { key ^= t.s1_tid_key[j]; offm_t ^= t.s1_tid_mid[j]; }
@@ -788,26 +836,20 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     const uint32_t c = ic.second;
                     // register bits [0, r1) must be group 1's canonical bits
                     if (((c >> s1.a) & ((1u << s1.r) - 1u)) != (uint32_t)(B & ((1 << s1.r) - 1))) return fail("tma2: step 1 register bits");
-                    uint32_t kk = key, offm = offm_t;
-                    for (int b = 0; b < 5; ++b) if ((B >> b) & 1) { kk ^= t.s1_reg_key[b]; offm ^= t.s1_reg_mid[b]; }
-                    if ((B >> s1.r) == 0 || true) {
-                        const uint32_t v = (c >> s2.a) & ((1u << s2.r) - 1u);
-                        // the kernel uses key bits from thread + batch bits only; group bits contribute 0
-                        uint32_t kb = key;
-                        for (int b = s1.r; b < 5; ++b) if ((B >> b) & 1) kb ^= t.s1_reg_key[b];
-                        if ((kb & 31u) != v) return fail("tma2: step 1 key (group 2 value)");
-                        if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
-                        for (int b = 0; b < s1.r; ++b) if (t.s1_reg_key[b]) return fail("tma2: group bit in key");
-                    }
-                    (void)kk;
+                    uint32_t offm = offm_t;
+                    for (int b = 0; b < 5; ++b) if ((B >> b) & 1) offm ^= t.s1_reg_mid[b];
+                    // the key comes from thread + batch bits only; group bits contribute 0
+                    uint32_t kb = key;
+                    for (int b = s1.r; b < 5; ++b) if ((B >> b) & 1) kb ^= t.s1_reg_key[b];
+                    if ((kb & 31u) != ((c >> s2.a) & ((1u << s2.r) - 1u))) return fail("tma2: step 1 key (group 2 value)");
+                    if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
                     if (offm & 7u) return fail("tma2: mid offset alignment");
                     const uint32_t slot = offm >> 3;
-                    const size_t gs = ((size_t)(pp ? (tid >> 8) : 0) << f) + slot;
-                    if (slot >= xslots || mid_canon[gs] != -1) return fail("tma2: exchange layout is not a bijection");
-                    mid_canon[gs] = (int)c;
+                    if (slot >= xslots || mid_canon[slot] != -1) return fail("tma2: exchange layout is not a bijection");
+                    mid_canon[slot] = (int)c;
                 }
-                // bank check: lanes 0-15 of every warp, same register, distinct 8-byte bank pairs
             }
+            // bank check: lanes 0-15 of every warp, same register, distinct 8-byte bank pairs
             for (int w = 0; w < nt / 16; ++w) {
                 for (int pass2 = 0; pass2 < 2; ++pass2) {
                     int banks = 0;
@@ -829,14 +871,17 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 }
                 if (banks != 0xFFFF) return fail("tma2: landing layout read with bank conflicts");
             }
+            auto st_index_of_addr = [&](int addr) {
+                for (int jj = 0; jj < f; ++jj) if (d.Fst[jj] == addr) return jj;
+                return -1;
+            };
             std::vector<char> seen_st((size_t)1 << f, 0);
             for (int tid = 0; tid < nt; ++tid) {
                 uint32_t key = 0, offm_t = 0;
                 uint32_t st_idx_t = 0;
                 for (int j = 0; j < lt; ++j) if ((tid >> j) & 1) {
                     key ^= t.s2_tid_key[j]; offm_t ^= t.s2_tid_mid[j];
-                    int found = -1;
-                    for (int jj = 0; jj < f; ++jj) if (d.F[jj] == t.s2_tid_addr[j]) found = jj;
+                    const int found = st_index_of_addr(t.s2_tid_addr[j]);
                     if (found < 0) return fail("tma2: store address bit outside the tile");
                     st_idx_t |= 1u << found;
                 }
@@ -845,16 +890,14 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     uint32_t kb = key;
                     for (int b = 0; b < 5; ++b) if ((B >> b) & 1) {
                         offm ^= t.s2_reg_mid[b];
-                        int found = -1;
-                        for (int jj = 0; jj < f; ++jj) if (d.F[jj] == t.s2_reg_addr[b]) found = jj;
+                        const int found = st_index_of_addr(t.s2_reg_addr[b]);
                         if (found < 0) return fail("tma2: store address bit outside the tile");
                         st_idx |= 1u << found;
                         if (b >= s2.r) kb ^= t.s2_reg_key[b];
                     }
                     const uint32_t slot = offm >> 3;
-                    const size_t gs = ((size_t)(pp ? (tid >> 8) : 0) << f) + slot;
-                    if (slot >= xslots || mid_canon[gs] < 0) return fail("tma2: step 2 reads an empty slot");
-                    const uint32_t c = (uint32_t)mid_canon[gs];
+                    if (slot >= xslots || mid_canon[slot] < 0) return fail("tma2: step 2 reads an empty slot");
+                    const uint32_t c = (uint32_t)mid_canon[slot];
                     if (((c >> s2.a) & ((1u << s2.r) - 1u)) != (uint32_t)(B & ((1 << s2.r) - 1))) return fail("tma2: step 2 register bits");
                     if ((kb & 31u) != ((c >> s1.a) & ((1u << s1.r) - 1u))) return fail("tma2: step 2 key (group 1 value)");
                     if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
@@ -866,10 +909,11 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     seen_st[st_idx] = 1;
                 }
             }
-            for (int j = 0; j < std::min<int>(t.tma_box[0], 3) && j < lt; ++j) if (t.s2_tid_addr[j] != d.F[j]) return fail("tma2: store lanes do not run along the hub");
+            for (int j = 0; j < std::min<int>(t.tma_box[0], 3) && j < lt; ++j) if (t.s2_tid_addr[j] != d.Fst[j] || d.Fst[j] != j) return fail("tma2: store lanes do not run along the hub");
             if (t.eb != s2.a || t.eb > 7) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
+            if (t.r1 != s1.r || t.r2 != s2.r) return fail("tma2: group sizes");
             // tensor-map dims: the box dims are disjoint runs that together are exactly F, dim 0 starts at
             // bit 0; every tile-index bit lies inside the span of a box-1 dim (its coordinate is the tile's
             // base address, which is zero on all tile bits, shifted down to the dim's lowest bit)
@@ -893,22 +937,25 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
             }
             for (int bit = 0; bit < n; ++bit)
                 if (!inF[bit] && !spanned[bit]) return fail("tma2: a tile-index bit is outside the tensor map");
-            const int a = n;
-            if (a != n || boxbits != f || t.tma_box[0] < 1) return fail("tma2: tensor map does not cover the state");
+            if (boxbits != f || t.tma_box[0] < 1) return fail("tma2: tensor map does not cover the state");
+        } else {
+            for (int j = 0; j < d.f; ++j)
+                if (d.F[j] != d.Fst[j]) return fail("store tile bits differ from load tile bits");
         }
         if (d.do_scale) ++nscaled;
         // permutation
-        std::vector<int> nq(qubit_at);
+        std::vector<int> nq2(qubit_at);
         for (int j = 0; j < d.f; ++j) {
-            // data on canonical bit st_canon[j] lands on address F[j]
-            nq[d.F[j]] = d.log_canon[d.st_canon[j]];
+            // data on canonical bit st_canon[j] lands on address Fst[j]
+            nq2[d.Fst[j]] = d.log_canon[d.st_canon[j]];
         }
+        if (d.xt) nq2[d.xt_st_addr] = d.xt_q;
         for (int i = 0; i < d.npair; ++i) {
             const int a = d.tile_addr[i], b = d.tile_addr[d.npair + i];
-            nq[a] = qubit_at[b];
-            nq[b] = qubit_at[a];
+            nq2[a] = qubit_at[b];
+            nq2[b] = qubit_at[a];
         }
-        qubit_at.swap(nq);
+        qubit_at.swap(nq2);
         ++pi;
     }
     if (next_qubit != -1) { *err = "self-check: not every qubit was processed"; return 5; }
@@ -919,19 +966,49 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
     return 0;
 }
 
+// Per pass, the contiguous sub-range [gate_first, gate_last] of the time-ordered gate list
+//   for t = n-1 .. 0:  H(q_t), CR_2(q_{t-1} -> q_t), ..., CR_{min(k,t)+1}(q_{t-min(k,t)} -> q_t);  then the swaps
+// that the pass folds ("the contiguous subrange of original gates folded into the block"), with the
+// number of Hadamards and controlled rotations in it.  The swaps are not gates of any pass: they are the
+// passes' store permutations.
+void qft_pass_gates(const QftHostPlan& plan, size_t pass, long long* n_h, long long* n_cr, long long* first,
+                    long long* last) {
+    const QftPassDesc& d = plan.passes[pass];
+    const int k = plan.k_eff;
+    *n_h = *n_cr = 0;
+    *first = *last = -1;
+    if (d.nsteps == 0) return;
+    const int t_hi = d.steps[0].t_hi;
+    const int t_lo = d.xt ? d.xt_q : d.win_lo;
+    long long idx = 0;
+    for (int t = plan.prm.n - 1; t > t_hi; --t) idx += 1 + std::min(k, t);
+    *first = idx;
+    for (int t = t_hi; t >= t_lo; --t) {
+        *n_h += 1;
+        *n_cr += std::min(k, t);
+    }
+    *last = idx + *n_h + *n_cr - 1;
+}
+
 std::string qft_describe_plan(const QftHostPlan& plan) {
     std::ostringstream o;
     o << "{\"n\":" << plan.prm.n << ",\"batch_bits\":" << plan.prm.batch_bits << ",\"k\":" << plan.k_eff << ",\"sign\":" << plan.prm.sign
       << ",\"norm\":" << plan.prm.norm << ",\"max_fused_qubits\":" << plan.prm.max_fused
       << ",\"tile_bits\":" << plan.tile_bits << ",\"hub_bits\":" << plan.hub_bits
-      << ",\"folded\":" << (plan.folded ? "true" : "false") << ",\"n_h\":" << plan.n_h << ",\"n_cr\":" << plan.n_cr
+      << ",\"folded\":" << (plan.folded ? "true" : "false") << ",\"ext_tile\":" << (plan.ext_tile ? "true" : "false")
+      << ",\"n_h\":" << plan.n_h << ",\"n_cr\":" << plan.n_cr
       << ",\"n_swap\":" << plan.n_swap << ",\"passes\":[";
     for (size_t i = 0; i < plan.passes.size(); ++i) {
         const QftPassDesc& d = plan.passes[i];
         if (i) o << ",";
-        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2PP ? "tma2pp" : d.kernel == QFT_KERNEL_TMA2 ? "tma2" : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic") << "\",\"tile_bits\":" << d.f
-          << ",\"F\":[";
-        for (int j = 0; j < d.f; ++j) o << (j ? "," : "") << (int)d.F[j];
+        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2 ? (d.xt ? "tma2x" : "tma2") : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic")
+          << "\",\"tile_bits\":" << d.f + d.xt << ",\"F\":[";
+        {
+            std::vector<int> F(d.F, d.F + d.f);
+            if (d.xt) F.push_back(d.xt_ld_addr);
+            std::sort(F.begin(), F.end());
+            for (size_t j = 0; j < F.size(); ++j) o << (j ? "," : "") << F[j];
+        }
         o << "],\"window\":[";
         bool first = true;
         for (int s = 0; s < d.nsteps; ++s)
@@ -939,17 +1016,24 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
                 o << (first ? "" : ",") << (int)d.steps[s].t_hi - q;
                 first = false;
             }
+        if (d.xt) o << "," << (int)d.xt_q;
         o << "],\"steps\":[";
         for (int s = 0; s < d.nsteps; ++s) o << (s ? "," : "") << (int)d.steps[s].r;
-        o << "],\"store_addr_of_canon\":[";
+        if (d.xt) o << ",1";
+        long long nh, ncr, g0, g1;
+        qft_pass_gates(plan, i, &nh, &ncr, &g0, &g1);
+        o << "],\"n_h\":" << nh << ",\"n_cr\":" << ncr << ",\"gate_first\":" << g0 << ",\"gate_last\":" << g1;
+        o << ",\"store_addr_of_canon\":[";
         {
             std::vector<int> sa(d.f);
-            for (int j = 0; j < d.f; ++j) sa[d.st_canon[j]] = d.F[j];
+            for (int j = 0; j < d.f; ++j) sa[d.st_canon[j]] = d.Fst[j];
             for (int c = 0; c < d.f; ++c) o << (c ? "," : "") << sa[c];
         }
         o << "],\"canon_qubits\":[";
         for (int c = 0; c < d.f; ++c) o << (c ? "," : "") << (int)d.log_canon[c];
-        o << "],\"pair_swaps\":[";
+        o << "]";
+        if (d.xt) o << ",\"ext\":{\"qubit\":" << (int)d.xt_q << ",\"load_addr\":" << (int)d.xt_ld_addr << ",\"store_addr\":" << (int)d.xt_st_addr << "}";
+        o << ",\"pair_swaps\":[";
         for (int p = 0; p < d.npair; ++p)
             o << (p ? "," : "") << "[" << (int)d.tile_addr[p] << "," << (int)d.tile_addr[d.npair + p] << "]";
         o << "],\"scale\":" << d.scale << ",\"bytes\":" << (16.0 * std::ldexp(1.0, plan.prm.n + plan.prm.batch_bits)) << "}";

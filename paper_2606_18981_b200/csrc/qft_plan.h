@@ -22,11 +22,10 @@
 #define QFT_MAX_TILEIDX_BITS 34
 #define QFT_MAX_STEPS 14
 #define QFT_MAX_RADIX_BITS 5
-// QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, 2 x 32 rows of end bases, one mbarrier, 5 coords
+// QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, 2 x 32 rows of end bases, one mbarrier,
+// 5 coords + the tensor-memory base address
 #define QFT_TMA2_MID_STRIDE 9   // float2 per row (<= 5 used; odd: rows of different lanes fall into different banks)
-#define QFT_TMA2_END_STRIDE 17  // float2 per row (R1 + R2 <= 10 used; odd for the same reason)
-// QFT_KERNEL_TMA2PP: 1 KB alignment slack + landing (2^14) + exchange (2^13) + mid + 4 end tables + mbarrier etc.
-#define QFT_TMA2PP_SMEM_BYTES (1024 + (8 << 14) + (8 << 13) + (32 * QFT_TMA2_MID_STRIDE + 4 * 32 * QFT_TMA2_END_STRIDE) * 8 + 8 + 48 + 8)
+#define QFT_TMA2_END_STRIDE 17  // float2 per row (R1 + R2 + 1 <= 11 used; odd for the same reason)
 #define QFT_TMA2_TABLE_BYTES(eb) ((32 * QFT_TMA2_MID_STRIDE + 2 * ((eb) > 5 ? (1 << (eb)) : 32) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)
 
 struct QftStep {
@@ -40,7 +39,6 @@ enum QftKernelKind : int32_t {
     QFT_KERNEL_GENERIC = 0,  // shared-memory staged tile pass, any descriptor
     QFT_KERNEL_FUSED2 = 1,   // two register steps: global -> reg -> smem -> reg -> global
     QFT_KERNEL_TMA2 = 2,     // persistent: TMA tile load -> reg -> smem -> reg -> global, packed FP32x2
-    QFT_KERNEL_TMA2PP = 3,   // tma2 on 2^14 tiles: two thread groups ping-pong on one exchange buffer
 };
 
 // QFT_KERNEL_TMA2 only.  Every shared-memory byte offset is a GF(2)-linear function of the thread
@@ -59,7 +57,6 @@ struct QftTma2Desc {
     int8_t t1_lo, t2_lo;                    // lowest logical qubit of group 1 / group 2
     int8_t r1, r2;
     int8_t tma_lo[5], tma_len[5], tma_box[5];  // tensor-map dims: address bits [lo, lo+len), box 2^box
-    int8_t pp;                                 // ping-pong variant: thread bit 8 = group bit, swizzled landing
     int8_t land_addr[16];                      // landing-index bit j of the shared-memory tile <-> address bit
 };
 
@@ -76,10 +73,20 @@ struct QftPassDesc {
     int32_t log2_threads;
     float scale;        // applied in the last step (1 unless this is the final pass)
     int32_t do_scale;
-    int32_t win_lo;     // lowest logical qubit of the window (-1: permutation-only pass)
-    int8_t F[16];         // load/store-order bit j <-> address bit F[j], ascending, F[j] = j for j < l
+    int32_t win_lo;     // lowest logical qubit the register steps process (-1: permutation-only pass)
+    // ---- tensor-memory extended tile (QFT_KERNEL_TMA2 only) ------------------------------------
+    // xt = 1: the pass owns tiles of 2^(f+1) amplitudes, F + {xt_ld_addr}.  A CTA runs the two halves
+    // (address bit xt_ld_addr = 0, then 1) through the register steps one after the other, parks the
+    // first half's results in tensor memory, and then applies the gates of one more qubit, xt_q =
+    // win_lo - 1 (H as a radix-2 butterfly between the halves and the controlled-R_m onto it from below),
+    // before it stores both halves; the butterfly's frequency bit lands on address bit xt_st_addr.
+    // The half-tile index bit is the LAST tile-index bit: tile_addr[ntile-1] = xt_ld_addr.
+    int32_t xt;
+    int8_t xt_q, xt_ld_addr, xt_st_addr, xt_pad;
+    int8_t F[16];         // load-order bit j <-> address bit F[j], ascending, F[j] = j for j < l
+    int8_t Fst[16];       // store-order bit j <-> address bit Fst[j], ascending (= F unless xt)
     int8_t ld_canon[16];  // load-order bit j  -> canonical bit
-    int8_t st_canon[16];  // store-order bit j -> canonical bit whose data lands on address F[j]
+    int8_t st_canon[16];  // store-order bit j -> canonical bit whose data lands on address Fst[j]
     int8_t log_canon[16]; // canonical bit -> logical qubit
     int8_t tile_addr[QFT_MAX_TILEIDX_BITS];  // tile-index bit -> address bit
     int8_t log_tile[QFT_MAX_TILEIDX_BITS];   // tile-index bit -> logical qubit held at load time
@@ -117,6 +124,7 @@ struct QftHostPlan {
     int k_eff = 0;  // min(k, n)
     int tile_bits = 0, hub_bits = 0, window = 0;
     bool folded = false;
+    bool ext_tile = false;  // some passes use the tensor-memory extended tile
     std::vector<QftPassDesc> passes;
     long long n_h = 0, n_cr = 0, n_swap = 0;
 };

@@ -18,6 +18,15 @@
 //   store  : straight from registers, lanes along the hub so every warp store covers whole granules,
 //            at the addresses the layout adapter dictates; for a pair pass into the
 //            partner tile after a cluster barrier (the partner's TMA load has completed by then).
+// Tensor-memory extended tiles (XT = 1, QftPassDesc::xt): the tile a CTA owns has 2^(F+1) amplitudes, one
+// address bit more than shared memory holds.  The CTA runs its two halves through steps 1 and 2 one after
+// the other; the first half's results wait in tensor memory (tcgen05.st, 64 words per thread: Blackwell's
+// 256 KB of TMEM per SM are otherwise idle in this kernel), and when the second half is in registers
+// each thread reads its own words back (tcgen05.ld) and applies the gates of one more qubit, the window's
+// lowest: H as a radix-2 butterfly between the halves, times the controlled-R_m onto it from the qubits
+// below the window (one factor per tile row e).  Both halves are then stored: the window grows by one
+// qubit, i.e. 11 qubits per pass with 128-byte granules or 10 with 256-byte granules, at 2^14-amplitude
+// shared-memory tiles.
 // Phase factors are never evaluated per amplitude: per CTA 32 x R1 "mid" bases, per tile 2^eb x (R1+R2)
 // "end" bases (sincos on an exact 32-bit fraction of a turn), multiplied up along the subset tree.
 #pragma once
@@ -58,6 +67,54 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, u
         "[%2];" ::"r"(smem_u32(dst)),
         "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
         : "memory");
+}
+
+// ---- tensor memory as a parking lot (XT) ----
+// 32x32b shape: thread i of a warp owns TMEM lane 32 (warp % 4) + i; .xN moves N consecutive columns
+// (32-bit words) of that lane to / from N registers.
+__device__ __forceinline__ void tmem_alloc(uint32_t* smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_dst)), "r"(ncols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+#define QFT_U(v) "r"(__float_as_uint(v))
+// park amplitudes x[BASE .. BASE+15] (32 words) at columns [taddr, taddr + 32)
+template <int BASE>
+__device__ __forceinline__ void tmem_park16(uint32_t taddr, const float2 (&x)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        QFT_U(x[BASE + 0].x), QFT_U(x[BASE + 0].y), QFT_U(x[BASE + 1].x), QFT_U(x[BASE + 1].y), QFT_U(x[BASE + 2].x),
+        QFT_U(x[BASE + 2].y), QFT_U(x[BASE + 3].x), QFT_U(x[BASE + 3].y), QFT_U(x[BASE + 4].x), QFT_U(x[BASE + 4].y),
+        QFT_U(x[BASE + 5].x), QFT_U(x[BASE + 5].y), QFT_U(x[BASE + 6].x), QFT_U(x[BASE + 6].y), QFT_U(x[BASE + 7].x),
+        QFT_U(x[BASE + 7].y), QFT_U(x[BASE + 8].x), QFT_U(x[BASE + 8].y), QFT_U(x[BASE + 9].x), QFT_U(x[BASE + 9].y),
+        QFT_U(x[BASE + 10].x), QFT_U(x[BASE + 10].y), QFT_U(x[BASE + 11].x), QFT_U(x[BASE + 11].y),
+        QFT_U(x[BASE + 12].x), QFT_U(x[BASE + 12].y), QFT_U(x[BASE + 13].x), QFT_U(x[BASE + 13].y),
+        QFT_U(x[BASE + 14].x), QFT_U(x[BASE + 14].y), QFT_U(x[BASE + 15].x), QFT_U(x[BASE + 15].y)
+        : "memory");
+}
+#undef QFT_U
+// fetch 8 parked amplitudes (16 words) from columns [taddr, taddr + 16)
+__device__ __forceinline__ void tmem_fetch8(uint32_t taddr, float2 (&p)[8]) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, "
+        "[%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+    // the registers are operands of the wait so that no consumer can be scheduled above it
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]),
+                   "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+                 :
+                 : "memory");
+#pragma unroll
+    for (int i = 0; i < 8; ++i) p[i] = make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1]));
 }
 
 // Plain C++ accesses (not asm): the compiler knows they touch shared memory, keeps them on the right
@@ -107,16 +164,17 @@ struct BatchApply {
     }
 };
 
-template <int R1, int R2, int KC, int LT>
+template <int R1, int R2, int KC, int LT, int XT>
 __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     qft_pass_tma2(float2* __restrict__ state, const __grid_constant__ CUtensorMap tmap,
                   const __grid_constant__ QftPassDesc d) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int F = LT + 5;
     constexpr int NT = 1 << LT;
+    constexpr int NQ = R1 + R2 + XT;  // columns of the end table: the window's qubits, lowest first ... and the extension's
     float2* midW = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F));
     uint64_t* mbar = reinterpret_cast<uint64_t*>(midW + 32 * kMidStride);
-    int* nextc = reinterpret_cast<int*>(mbar + 1);           // next tile's TMA coordinates (5 ints, padded to 6)
+    int* nextc = reinterpret_cast<int*>(mbar + 1);           // next tile's TMA coordinates (5 ints) + the TMEM base address
     float2* endW = reinterpret_cast<float2*>(nextc + 6);     // two end tables (by parity) of max(32, 2^eb) rows
     const uint32_t tid = threadIdx.x;
     const QftTma2Desc& t = d.tma;
@@ -148,6 +206,12 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         mbar_init(mbar, 1);
         fence_proxy_async();
     }
+    uint32_t tpark = 0;  // this warp's parking columns in tensor memory
+    constexpr uint32_t kTmemCols = (NT / 128) * 64;
+    if constexpr (XT) {
+        if (tid < 32) tmem_alloc(reinterpret_cast<uint32_t*>(nextc + 5), kTmemCols);
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
     // mid bases: midW[u1][b] = the phase that group 2's b-th qubit (when set) contributes to an amplitude
     // whose group-1 frequency bits are u1: the product over the set bits i of u1 of the controlled-R_m
     // from that qubit onto group 1's i-th qubit (phases add exactly as 32-bit fractions of a turn)
@@ -160,19 +224,26 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         midW[u1 * kMidStride + b] = qftp::cis_fwd_u32(ph);
     }
     __syncthreads();
+    if constexpr (XT) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t warp = tid >> 5;
+        tpark = *reinterpret_cast<volatile uint32_t*>(nextc + 5) + (((warp & 3u) * 32u) << 16) + (warp >> 2) * 64u;
+    }
 
     // ---- tile walk ----
     const uint32_t csz = d.npair ? 2u : 1u;
     const uint32_t rho = d.npair ? (blockIdx.x & 1u) : 0u;
-    const uint32_t nunits = (1u << d.ntile) / csz;
+    const int nbig = d.ntile - XT;  // index bits of the tiles a CTA owns (an extended tile = two half-tiles)
+    const uint32_t nunits = (1u << nbig) / csz;
     const uint32_t ustride = gridDim.x / csz;
     const bool has_end = win_lo > 0;
     const uint32_t end_rows = t.eb > 5 ? (1u << t.eb) : 32u;
 
-    // tile index -> TMA coordinates (HBM address bits of the tile, cut into the tensor map's dims)
-    auto coords_of = [&](uint32_t un, int (&c)[5]) {
+    // tile index (+ half) -> TMA coordinates (HBM address bits of the tile, cut into the tensor map's dims)
+    auto coords_of = [&](uint32_t un, uint32_t half, int (&c)[5]) {
         uint32_t ml, ms;
         decode_tile(un * csz + rho, d.npair, &ml, &ms);
+        ml |= half << nbig;
         uint64_t base = 0;
         for (int i = 0; i < d.ntile; ++i)
             if ((ml >> i) & 1u) base |= 1ull << d.tile_addr[i];
@@ -186,40 +257,51 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     uint32_t unit = blockIdx.x / csz;
     if (unit < nunits && tid == 0) {
         int c[5];
-        coords_of(unit, c);
+        coords_of(unit, 0u, c);
         mbar_expect_tx(mbar, 8u << F);
         tma_load_5d(smem_raw, &tmap, mbar, c[0], c[1], c[2], c[3], c[4]);
     }
     uint32_t parity = 0;
     for (; unit < nunits; unit += ustride) {
+#pragma unroll 1
+        for (uint32_t half = 0; half <= (uint32_t)XT; ++half) {
         // ---- bookkeeping while the tile's load is in flight (few registers live here) ----
+        const bool last_half = half == (uint32_t)XT;
+        const bool has_next = !last_half || unit + ustride < nunits;
         uint64_t base_st = 0;
         float2* endWp = endW + parity * (end_rows * kEndStride);
         {
             uint32_t ml, ms;
             decode_tile(unit * csz + rho, d.npair, &ml, &ms);
+            ml |= half << nbig;
             uint64_t Ltile = 0;
-            for (int i = 0; i < d.ntile; ++i) {
+            for (int i = 0; i < d.ntile; ++i)
                 if ((ml >> i) & 1u) Ltile |= 1ull << d.log_tile[i];
+            for (int i = 0; i < nbig; ++i)
                 if ((ms >> i) & 1u) base_st |= 1ull << d.tile_addr[i];
-            }
             if (has_end) {
                 // end bases of this tile: endW[e][q] = product of the controlled-R_m from every qubit
-                // below the window (tile-index bits + in-tile bits e) onto the window's q-th qubit
-                const uint32_t nq = R1 + R2;
-                const uint32_t cnt = nq << t.eb;
+                // below the window (tile-index bits + in-tile bits e) onto the window's q-th qubit; with
+                // an extended tile the last column belongs to the extension's qubit win_lo - 1
+                const uint32_t cnt = (uint32_t)NQ << t.eb;
                 for (uint32_t i = tid; i < cnt; i += NT) {
-                    const uint32_t e = i / nq, q = i % nq;
+                    const uint32_t e = i / NQ, q = i % NQ;
                     uint64_t L = Ltile;
                     for (int b = 0; b < t.eb; ++b)
                         if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
                     L &= lbmask;
-                    endWp[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, win_lo + (int)q, k));
+                    int tq = win_lo + (int)q;
+                    if (XT && q == (uint32_t)(R1 + R2)) {
+                        tq = win_lo - 1;
+                        L &= (1ull << tq) - 1ull;
+                    }
+                    endWp[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, tq, k));
                 }
             }
-            if (tid == 0 && unit + ustride < nunits) {
+            if (tid == 0 && has_next) {
                 int c[5];
-                coords_of(unit + ustride, c);
+                if (last_half) coords_of(unit + ustride, 0u, c);
+                else coords_of(unit, half + 1u, c);
 #pragma unroll
                 for (int j = 0; j < 5; ++j) nextc[j] = c[j];
             }
@@ -229,7 +311,8 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         // spill): one XOR next to each access is cheaper than a local-memory reload
         asm volatile("" : "+r"(off1_ld), "+r"(off1_mid), "+r"(off2_mid));
         mbar_wait(mbar, parity);
-        if (d.npair) cluster_arrive_relaxed();  // this CTA's tile is on chip: the partner may overwrite it in HBM
+        // this CTA's whole tile is on chip (or in registers / tensor memory): the partner may overwrite it in HBM
+        if (d.npair && last_half) cluster_arrive_relaxed();
 
         // ------------------------------ step 1 ------------------------------
 #define QFT_LD1(B) x[B] = lds64(smem_raw, off1_ld ^ reg_off<B>(c1ld));
@@ -255,7 +338,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
 #undef QFT_LD2
         fence_proxy_async();
         __syncthreads();  // the buffer is free again
-        if (tid == 0 && unit + ustride < nunits) {
+        if (tid == 0 && has_next) {
             // prefetch the next tile while this one is transformed and stored
             mbar_expect_tx(mbar, 8u << F);
             tma_load_5d(smem_raw, &tmap, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
@@ -281,8 +364,8 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
             BatchApply<R2, 0, NBM, false>::run(x, WM, one);
         }
         qftp::dif_group<5, R2, KC>(x);
+        constexpr int NB2 = 1 << (5 - R2);
         if (has_end) {
-            constexpr int NB2 = 1 << (5 - R2);
             float2 W2[NB2][5];
             float2 cfac[NB2];
 #pragma unroll
@@ -308,23 +391,75 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
 #pragma unroll
             for (int B = 0; B < 32; ++B) x[B] = qftp::cscale(x[B], d.scale);
         }
-        if (d.conj) {
-#pragma unroll
-            for (int B = 0; B < 32; ++B) x[B].y = -x[B].y;
+        if constexpr (XT) {
+            if (!last_half) {
+                // first half: park the results in tensor memory until the second half has caught up
+                tmem_park16<0>(tpark, x);
+                tmem_park16<16>(tpark + 32u, x);
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                parity ^= 1u;
+                continue;
+            }
         }
-        if (d.npair) cluster_wait();  // the partner holds its tile on chip: its addresses may be overwritten
         float2* __restrict__ dst = state + (base_st | st_thread);
+        if constexpr (XT) {
+            // H on the extension's qubit: butterfly between the parked half (bit = 0) and this one (bit = 1), then
+            // the controlled-R_m onto it from the qubits below the window; the frequency
+            // bit lands on address bit xt_st_addr
+            float2 wg[NB2];
 #pragma unroll
-        for (int B = 0; B < 32; ++B) {
-            uint64_t o = 0;
+            for (int bt = 0; bt < NB2; ++bt) {
+                uint32_t kk = key2;
 #pragma unroll
-            for (int b = 0; b < 5; ++b)
-                if (B & (1 << b)) o += c2st[b];
-            dst[o] = x[B];
+                for (int i = 0; i < 5 - R2; ++i)
+                    if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
+                wg[bt] = endWp[((kk >> 8) & 127u) * kEndStride + (R1 + R2)];
+            }
+            if (d.npair) cluster_wait();  // the partner holds its tile on chip: its addresses may be overwritten
+            float2* __restrict__ dst1 = dst + (1ull << d.xt_st_addr);
+#pragma unroll
+            for (int c8 = 0; c8 < 4; ++c8) {
+                float2 pk[8];
+                tmem_fetch8(tpark + 16u * c8, pk);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int B = 8 * c8 + i;
+                    float2 lo = qftp::padd(pk[i], x[B]);
+                    float2 hi = qftp::cmul(qftp::psub(pk[i], x[B]), wg[B >> R2]);
+                    if (d.conj) { lo.y = -lo.y; hi.y = -hi.y; }
+                    uint64_t o = 0;
+#pragma unroll
+                    for (int b = 0; b < 5; ++b)
+                        if (B & (1 << b)) o += c2st[b];
+                    dst[o] = lo;
+                    dst1[o] = hi;
+                }
+            }
+        } else {
+            if (d.conj) {
+#pragma unroll
+                for (int B = 0; B < 32; ++B) x[B].y = -x[B].y;
+            }
+            if (d.npair) cluster_wait();  // the partner holds its tile on chip: its addresses may be overwritten
+#pragma unroll
+            for (int B = 0; B < 32; ++B) {
+                uint64_t o = 0;
+#pragma unroll
+                for (int b = 0; b < 5; ++b)
+                    if (B & (1 << b)) o += c2st[b];
+                dst[o] = x[B];
+            }
         }
         parity ^= 1u;
+        }
     }
 #undef QFT_ALL32
+    if constexpr (XT) {
+        // every thread's tensor-memory traffic has completed (wait::ld / wait::st above): give the columns back
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid < 32) tmem_dealloc(*reinterpret_cast<volatile uint32_t*>(nextc + 5), kTmemCols);
+    }
 }
 
 }  // namespace qftk

@@ -4,27 +4,27 @@
 
 typedef void (*tma2_kernel_t)(float2*, const CUtensorMap, const QftPassDesc);
 
-template <int R1, int R2, int LT>
+template <int R1, int R2, int LT, int XT>
 static tma2_kernel_t qft_pick_tma2_kc(int kc) {
     switch (kc) {
-        case 0: return qftk::qft_pass_tma2<R1, R2, 0, LT>;
-        case 1: return qftk::qft_pass_tma2<R1, R2, 1, LT>;
-        case 2: return qftk::qft_pass_tma2<R1, R2, 2, LT>;
-        case 3: return qftk::qft_pass_tma2<R1, R2, 3, LT>;
-        default: return qftk::qft_pass_tma2<R1, R2, 4, LT>;
+        case 0: return qftk::qft_pass_tma2<R1, R2, 0, LT, XT>;
+        case 1: return qftk::qft_pass_tma2<R1, R2, 1, LT, XT>;
+        case 2: return qftk::qft_pass_tma2<R1, R2, 2, LT, XT>;
+        case 3: return qftk::qft_pass_tma2<R1, R2, 3, LT, XT>;
+        default: return qftk::qft_pass_tma2<R1, R2, 4, LT, XT>;
     }
 }
 
-#define QFT_TMA2_DEFINE_PICK(LT)                                          \
-    tma2_kernel_t qft_pick_tma2_lt##LT(int r1, int r2, int kc) {          \
-        if (r1 == 5 && r2 == 5) return qft_pick_tma2_kc<5, 5, LT>(kc);    \
-        if (r1 == 5 && r2 == 4) return qft_pick_tma2_kc<5, 4, LT>(kc);    \
-        if (r1 == 4 && r2 == 4) return qft_pick_tma2_kc<4, 4, LT>(kc);    \
-        if (r1 == 4 && r2 == 3) return qft_pick_tma2_kc<4, 3, LT>(kc);    \
-        if (r1 == 3 && r2 == 3) return qft_pick_tma2_kc<3, 3, LT>(kc);    \
-        if (r1 == 3 && r2 == 2) return qft_pick_tma2_kc<3, 2, LT>(kc);    \
-        if (r1 == 2 && r2 == 2) return qft_pick_tma2_kc<2, 2, LT>(kc);    \
-        if (r1 == 2 && r2 == 1) return qft_pick_tma2_kc<2, 1, LT>(kc);    \
-        if (r1 == 1 && r2 == 1) return qft_pick_tma2_kc<1, 1, LT>(kc);    \
-        return nullptr;                                                   \
+#define QFT_TMA2_DEFINE_PICK(LT)                                             \
+    tma2_kernel_t qft_pick_tma2_lt##LT(int r1, int r2, int kc) {             \
+        if (r1 == 5 && r2 == 5) return qft_pick_tma2_kc<5, 5, LT, 0>(kc);    \
+        if (r1 == 5 && r2 == 4) return qft_pick_tma2_kc<5, 4, LT, 0>(kc);    \
+        if (r1 == 4 && r2 == 4) return qft_pick_tma2_kc<4, 4, LT, 0>(kc);    \
+        if (r1 == 4 && r2 == 3) return qft_pick_tma2_kc<4, 3, LT, 0>(kc);    \
+        if (r1 == 3 && r2 == 3) return qft_pick_tma2_kc<3, 3, LT, 0>(kc);    \
+        if (r1 == 3 && r2 == 2) return qft_pick_tma2_kc<3, 2, LT, 0>(kc);    \
+        if (r1 == 2 && r2 == 2) return qft_pick_tma2_kc<2, 2, LT, 0>(kc);    \
+        if (r1 == 2 && r2 == 1) return qft_pick_tma2_kc<2, 1, LT, 0>(kc);    \
+        if (r1 == 1 && r2 == 1) return qft_pick_tma2_kc<1, 1, LT, 0>(kc);    \
+        return nullptr;                                                      \
     }

@@ -8,7 +8,9 @@ tests/test_large_checks_cpu.py pin against the gate-by-gate oracle at small n on
                          element (oracle.orc_element_turns) summed over the whole input:
                          turns_k(K, j) = sign * sum_{t : y_t = 1} tr_{k,t}(j) / 2^{t+1},
                          y_t = bit n-1-t of K, tr_{k,t}(j) = (j mod 2^{t+1}) with bits below t-k
-                         cleared.  For k >= n-1 this is the DFT phase sign * (j K mod N) / N.
+                         cleared.  For k >= n-1 this is the DFT phase sign * (j K mod N) / N.  The
+                         phase is linear in the bits of j, so it factors into a low-bits and a
+                         high-bits table and the sums for all sampled K are two matrix products.
   tones_closed_form()    AQFT_k of a sum of tones, every output, by factorising over input bits:
                          out[K] = sum_i a_i prod_c (1 + exp(2 pi i alpha_c)) / 2,
                          alpha_c = f_i 2^c / N - field_c(K) / 2^{k+1}.
@@ -38,35 +40,61 @@ def norm2(x: torch.Tensor, chunk_bits: int = 26) -> float:
     return float(acc.item())
 
 
+def _phase_coefficients(n: int, Ks, k: int, sign: int) -> torch.Tensor:
+    """c[b, s]: the turns that input bit b contributes to the matrix element <Ks[s]| AQFT_k |j>.
+
+    turns_k(K, j) = sign * sum_{t : y_t = 1} tr_{k,t}(j) / 2^{t+1} is linear in the bits of j: bit b belongs to
+    tr_{k,t}(j) iff t - k <= b <= t, so c_b = sign * sum_{t = b}^{min(n-1, b+k)} y_t 2^{b-t-1}, y_t = bit n-1-t
+    of K.  Every term is a dyadic rational >= 2^-(k+1): sums of them are exact in float64."""
+    c = torch.zeros(n, len(Ks), dtype=torch.float64)
+    for s, K in enumerate(Ks):
+        K = int(K)
+        for b in range(n):
+            acc = 0.0
+            for t in range(b, min(n - 1, b + k) + 1):
+                if (K >> (n - 1 - t)) & 1:
+                    acc += 2.0 ** (b - t - 1)
+            c[b, s] = sign * acc
+    return c
+
+
+def _cis_turns(turns: torch.Tensor) -> torch.Tensor:
+    fr = turns - torch.floor(turns)  # exact: the turns are dyadic rationals well inside float64
+    ang = fr * (2.0 * math.pi)
+    return torch.complex(torch.cos(ang), torch.sin(ang))
+
+
+def _bits(idx: torch.Tensor, nbits: int) -> torch.Tensor:
+    sh = torch.arange(nbits, dtype=torch.int64, device=idx.device)
+    return ((idx[:, None] >> sh[None, :]) & 1).to(torch.float64)
+
+
 def sampled_outputs(x: torch.Tensor, Ks, k: int, sign: int = -1, chunk_bits: int = 24) -> torch.Tensor:
-    """Direct float64 sums for the output indices Ks (unitary scaling); x is the INPUT state."""
+    """Direct float64 sums for the output indices Ks (unitary scaling); x is the INPUT state.
+
+    out[K] = 2^{-n/2} sum_j x[j] exp(2 pi i turns_k(K, j)).  Because turns_k is linear in the bits of j
+    (_phase_coefficients), the phase factorises over j = j_hi 2^h + j_lo into W_hi[j_hi] W_lo[j_lo], so the sum is
+    W_hi^T (X W_lo) with X the input seen as a 2^(n-h) x 2^h matrix: one complex128 matrix product per chunk of rows
+    for all sampled indices at once.  Exact k (k >= n-1) needs no special case: then c_b = sign K 2^b / N mod 1."""
     N = x.numel()
     n = int(N).bit_length() - 1
     cb, C, nc = _chunks(n, chunk_bits)
+    h = min(cb, 12)
     dev = x.device
-    base = torch.arange(C, dtype=torch.int64, device=dev)
+    c = _phase_coefficients(n, Ks, min(k, n), sign).to(dev)
+    lo = torch.arange(1 << h, dtype=torch.int64, device=dev)
+    W_lo = _cis_turns(_bits(lo, h) @ c[:h]) if h > 0 else torch.ones(1, len(Ks), dtype=torch.complex128, device=dev)
+    R = C >> h  # rows per chunk
+    rows = torch.arange(R, dtype=torch.int64, device=dev)
     out = torch.zeros(len(Ks), dtype=torch.complex128, device=dev)
-    exact = k >= n - 1
-    for c in range(nc):
-        j = base + c * C
-        xc = x[c * C:(c + 1) * C].to(torch.complex128)
-        for s, K in enumerate(Ks):
-            K = int(K)
-            if exact:
-                p = (j * K) & (N - 1)  # int64 wrap-around is exact modulo 2^n
-                turns = p.to(torch.float64) * (float(sign) / N)
-            else:
-                turns = torch.zeros(C, dtype=torch.float64, device=dev)
-                for t in range(n):
-                    if not (K >> (n - 1 - t)) & 1:
-                        continue
-                    tr = j & ((1 << (t + 1)) - 1)
-                    if t - k > 0:
-                        tr = tr & ~((1 << (t - k)) - 1)
-                    turns += tr.to(torch.float64) * (float(sign) / float(1 << (t + 1)))
-            ang = turns * (2.0 * math.pi)
-            w = torch.complex(torch.cos(ang), torch.sin(ang))
-            out[s] += (xc * w).sum()
+    for ci in range(nc):
+        X = x[ci * C:(ci + 1) * C].view(R, 1 << h).to(torch.complex128)
+        P = X @ W_lo  # [R, S]
+        if n > h:
+            W_hi = _cis_turns(_bits(rows + ci * R, n - h) @ c[h:])
+            out += (P * W_hi).sum(dim=0)
+        else:
+            out += P.sum(dim=0)
     return out * (2.0 ** (-0.5 * n))
 
 

@@ -133,25 +133,3 @@ def test_execute_is_cuda_graph_capturable():
     got = t.cpu().numpy().astype(np.complex128)
     assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 2e-5
     plan.close()
-
-
-@pytest.mark.parametrize("n", [23, 25])
-def test_pingpong_variant_against_oracle(n):
-    """QFT_FLAG_PINGPONG (opt-in, tile_bits = 14): two thread groups sharing one exchange buffer, 128B-swizzled
-    landing buffer.  Slower than the default kernel (profiles/r01_tile_hub_sweep.md) but kept correct."""
-    import torch
-
-    import paper_2606_18981_b200 as qft
-
-    x = qi.gaussian(n, n)
-    for k, sign in ((n, -1), (3, 1)):
-        plan = qft.Plan(n, k, 13, sign, 0, 14, 4, qft.QFT_FLAG_PINGPONG)
-        plan.self_check()
-        assert "tma2pp" in [p["kernel"] for p in plan.describe()["passes"]]
-        t = torch.from_numpy(x).cuda()
-        plan.execute(t)
-        torch.cuda.synchronize()
-        plan.close()
-        ref = oracle.qft(x, k, sign, 0)
-        got = t.cpu().numpy().astype(np.complex128)
-        assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 1e-4

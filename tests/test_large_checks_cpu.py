@@ -21,6 +21,29 @@ def test_sampled_outputs_match_oracle(k):
         assert np.max(np.abs(got - oracle.outputs_at(x, Ks, k, sign))) < 1e-12
 
 
+@pytest.mark.parametrize("n,k", [(14, 5), (14, 14), (13, 0), (9, 2), (3, 1)])
+def test_sampled_outputs_32_indices_both_tables(n, k):
+    """Sizes at which both the low-bits and the high-bits phase table are in play (h = 12 or chunk_bits < n),
+    32 sampled indices at once as in the n = 30 / 33 GPU tests, against the full oracle output."""
+    x = qi.gaussian(n, 40 + n)
+    rng = np.random.default_rng(n)
+    Ks = sorted({int(v) for v in rng.integers(0, 1 << n, size=64)})[:32]
+    full = oracle.qft(x, k)
+    for chunk_bits in (24, max(1, n - 3)):
+        got = lc.sampled_outputs(torch.from_numpy(x), Ks, k, -1, chunk_bits=chunk_bits).numpy()
+        assert np.max(np.abs(got - full[Ks])) < 1e-12
+
+
+def test_phase_coefficients_reduce_to_the_dft_for_exact_k():
+    """Exact k: the linear phase must be K j / N, i.e. c_b = -K 2^b / N modulo one turn."""
+    n = 11
+    for K in (0, 1, 2, 777, 2047):
+        c = lc._phase_coefficients(n, [K], n, -1)[:, 0].numpy()
+        for b in range(n):
+            want = (-(K << b) / (1 << n)) % 1.0
+            assert abs((c[b] % 1.0) - want) < 1e-15
+
+
 @pytest.mark.parametrize("k", [0, 1, 4, 8, 10, 11, 30])
 def test_tones_closed_form_matches_oracle(k):
     n = 11

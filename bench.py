@@ -12,8 +12,13 @@ The state is far larger than the 126 MB L2, so no L2 flush is needed between ite
 With N > 1 (torchrun) every rank transforms its own state (replicas only: the path does not shard,
 DESIGN.md section "multi-GPU"); value = all ranks' work / max-over-ranks time, "scaling": "weak".
 
---impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample
-of the same workload; see DESIGN.md "measurement".
+The default run also times, briefly, n = 26 and n = 33 and one batched shape ("sweep" / "batched" in the
+JSON line, each with its own fraction of the HBM roofline), and the CPU oracle on whole circuits at
+n = 22 and n = 26 ("cpu_baseline").
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores: every step is one WHOLE
+gate-by-gate circuit at the largest n <= 26 for which steps + warmup circuits fit the time budget (a bounded
+sample of the n = 30 workload: same circuit family, smaller state); see DESIGN.md "measurement".
 """
 from __future__ import annotations
 
@@ -44,9 +49,11 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", default="", help="comma list of extra n to time briefly, e.g. 20,22,26,33")
-    ap.add_argument("--batched", default="", help="comma list of n:log2_batch pairs to time briefly (batched plans), "
-                                                  "e.g. 10:18,16:12")
+    ap.add_argument("--extrapolate-cpu", action="store_true",
+                    help="also estimate the oracle's time at the bench n from a few gates (labelled as extrapolated)")
+    ap.add_argument("--sweep", default="26,33", help="comma list of extra n to time briefly ('' = none)")
+    ap.add_argument("--batched", default="16:12", help="comma list of n:log2_batch pairs to time briefly (batched "
+                                                       "plans; '' = none), e.g. 10:18,16:12")
     return ap.parse_args()
 
 
@@ -188,9 +195,27 @@ def time_config(qft, torch, n, k, args, steps, warmup, per_pass=True, log2_batch
     return res
 
 
+def oracle_full(n, k, warmup=1, trials=3):
+    """Time the oracle's WHOLE gate-by-gate circuit (every H, controlled-R_m and swap, fp64) on a seeded
+    Gaussian state of 2^n amplitudes: `warmup` untimed runs, then `trials` timed ones.  Returns (times, cores)."""
+    import oracle
+    import qft_inputs as qi
+
+    x = qi.gaussian(n, 1)
+    for _ in range(warmup):
+        oracle.qft(x, n if k is None else k)
+    times = []
+    for _ in range(trials):
+        t0 = time.perf_counter()
+        oracle.qft(x, n if k is None else k)
+        times.append(time.perf_counter() - t0)
+    return times, oracle.max_threads()
+
+
 def oracle_sample(n, k, reps=1):
-    """Time a bounded sample of the oracle's gate-by-gate circuit on the full 2^n fp64 state and
-    extrapolate to the whole circuit: t = n_H t_H + n_CR t_CR + n_SWAP t_SWAP."""
+    """EXTRAPOLATION, reported only as a labelled extra: time a few gates of the n-qubit circuit on the full 2^n fp64
+    state (H, controlled-R_m and SWAP at low, middle and high qubit positions) and scale by gate type:
+    t = n_H t_H + n_CR t_CR + n_SWAP t_SWAP."""
     import numpy as np
 
     import oracle
@@ -204,7 +229,8 @@ def oracle_sample(n, k, reps=1):
     hs = [g for g in gates if g[0] == oracle.GATE_H]
     crs = [g for g in gates if g[0] == oracle.GATE_CR]
     sws = [g for g in gates if g[0] == oracle.GATE_SWAP]
-    sample = [hs[0], hs[-1]] + ([crs[0], crs[len(crs) // 2]] if crs else []) + (sws[:1] if sws else [])
+    pick = lambda v: [v[0], v[len(v) // 2], v[-1]] if len(v) >= 3 else list(v)
+    sample = pick(hs) + pick(crs) + pick(sws)[:2]
     t = {0: [], 1: [], 2: []}
     for _ in range(reps):
         for g in sample:
@@ -214,9 +240,8 @@ def oracle_sample(n, k, reps=1):
     mean = lambda v: sum(v) / len(v) if v else 0.0
     est = n_h * mean(t[0]) + n_cr * mean(t[1]) + n_sw * mean(t[2])
     spent = sum(sum(v) for v in t.values())
-    desc = (f"{len(sample)} of the {len(gates)} gates of the n={n} circuit (H q{int(hs[0][1])}, H q{int(hs[-1][1])}, "
-            f"2 CR, 1 SWAP) on the full 2^{n} fp64 state; whole-circuit time extrapolated as "
-            f"n_H*t_H + n_CR*t_CR + n_SWAP*t_SWAP = {est:.1f} s ({spent:.1f} s measured)")
+    desc = (f"EXTRAPOLATED from {len(sample)} of the {len(gates)} gates of the n={n} circuit on the full 2^{n} fp64 "
+            f"state as n_H*t_H + n_CR*t_CR + n_SWAP*t_SWAP = {est:.1f} s ({spent:.1f} s measured)")
     return est, spent, desc, oracle.max_threads()
 
 
@@ -232,33 +257,40 @@ def run_reference(args):
     if rank != 0:
         return 0
     n = args.n
-    flops = 5.0 * (1 << n) * n
-    # keep the whole run within a few minutes: the per-step sample is ~5 gates on the full state
-    n_eff = n
     steps, warmup = max(1, args.steps), max(0, args.warmup)
-    budget_steps = 3
-    steps_run = min(steps, budget_steps)
-    warm_run = min(warmup, 1)
-    vals = []
-    desc = ""
-    cores = 1
-    for i in range(warm_run + steps_run):
-        est, spent, desc, cores = oracle_sample(n_eff, args.k)
-        if i >= warm_run:
-            vals.append(est)
-    est = sorted(vals)[len(vals) // 2]
-    gf = flops / est / 1e9
+    # Every step = one whole oracle circuit.  The n = 30 workload itself (16 GiB of fp64 state, minutes per circuit)
+    # does not fit `steps + warmup` circuits into a few minutes, so the step is a bounded sample of it: the same
+    # circuit on a 2^n_eff state, n_eff the largest of 26, 24, 22, 20 whose projected total stays under the budget.
+    budget_s = 200.0
+    n_eff, probe = None, None
+    for cand in (26, 24, 22, 20):
+        if cand > n:
+            continue
+        tt, cores = oracle_full(cand, args.k, warmup=0, trials=1)
+        n_eff, probe = cand, tt[0]
+        if probe * (steps + warmup) <= budget_s:
+            break
+    if n_eff is None:
+        n_eff = n
+    warm_left = max(0, warmup - 1)  # the probe was the first warm-up
+    times, cores = oracle_full(n_eff, args.k, warmup=warm_left, trials=steps)
+    t_step = sum(times) / len(times)
+    flops = 5.0 * (1 << n_eff) * n_eff
+    gf = flops / t_step / 1e9
+    med = sorted(times)[len(times) // 2]
+    sample = (f"{steps} timed + {warmup} warm-up WHOLE gate-by-gate oracle circuits (fp64, OpenMP) at n={n_eff} instead of "
+              f"n={n}: the largest state for which that many circuits fit {budget_s:.0f} s; mean {t_step:.3f} s, "
+              f"median {med:.3f} s per circuit; GFLOP/s = 5 N log2 N / t at n={n_eff}")
     line = {
         "impl": "reference", "metric": "dft_equiv_gflops", "value": gf, "unit": "GFLOP/s", "n_gpus": args.gpus,
-        "steps": steps_run, "warmup": warm_run, "ms_per_step": est * 1e3, "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_text(n, args.k), "n_qubits": n,
                    "aqft_cutoff_k": n if args.k is None else min(args.k, n),
-                   "implementation": "CPU oracle (gate-by-gate fp64, OpenMP), bounded sample per step"},
-        "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": desc},
+                   "implementation": "CPU oracle (gate-by-gate fp64, OpenMP)", "sample_n_qubits": n_eff},
+        "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": gf, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
-        "note": f"requested steps={steps} warmup={warmup}; ran {steps_run}+{warm_run} bounded samples",
     }
     print(json.dumps(line))
     return 0
@@ -343,18 +375,21 @@ def main():
     dom_ms = sum(share[dom]) / len(share[dom])
     bytes_per_launch = 16.0 * N  # 8 B read + 8 B written per amplitude per pass
     achieved = bytes_per_launch / (dom_ms * 1e-3) / 1e9
-    traffic = None
+    # measured DRAM bytes per launch of the dominant kernel: a COPY of the figure in the committed ncu --set full
+    # capture (profiles/r02_traffic.csv: n, kernel, bytes), null when that file has no row for this (n, kernel)
+    traffic, traffic_source = None, None
     try:
-        # measured DRAM bytes per launch of the dominant kernel, from the committed ncu --set full capture
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as fh:
             for row in fh:
                 f = [v.strip() for v in row.split(",")]
                 if len(f) >= 3 and f[0] == str(n) and f[1] == dom:
                     traffic = float(f[2])
+                    traffic_source = ("profiles/r02_traffic.csv (dram__bytes_read.sum + dram__bytes_write.sum of one "
+                                      "ncu --set full capture of this kernel at this n; not re-measured in this run)")
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_src,
                 "bytes_per_launch": bytes_per_launch, "launch_ms": dom_ms,
                 "pass_ms": pass_ms, "pass_kernels": kernels,
                 "step_gbs": npass * bytes_per_launch / (ms_per_step * 1e-3) / 1e9,
@@ -386,23 +421,34 @@ def main():
 
     # ---- optional brief sweep over other n (reported, not the headline) ----
     sweep = []
-    if args.sweep and rank == 0:
+    if args.sweep and rank == 0 and world == 1:
         del state
         plan.close()
         torch.cuda.empty_cache()
         for sn in [int(v) for v in args.sweep.split(",") if v]:
+            if sn == n:
+                continue
+            free, _ = torch.cuda.mem_get_info()
+            if 8 * (1 << sn) * 1.05 > free:
+                sweep.append({"n": sn, "skipped": "not enough free device memory"})
+                continue
             st = 5 if sn >= 32 else 10
             r = time_config(qft, torch, sn, None, args, st, 3, per_pass=True)
-            sweep.append({"n": sn, "passes": r["passes"], "median_ms": r["median_ms"],
+            gbs = r["passes"] * 16.0 * (1 << sn) / (r["median_ms"] * 1e-3) / 1e9
+            kinds = [p["kernel"] for p in r["plan"].describe()["passes"]]
+            slow = max(r["pass_ms"])
+            sweep.append({"n": sn, "passes": r["passes"], "ideal_passes": math.ceil(sn / 13), "steps": st,
+                          "median_ms": r["median_ms"],
                           "gflops": 5.0 * (1 << sn) * sn / (r["median_ms"] * 1e-3) / 1e9,
-                          "gbs": r["passes"] * 16.0 * (1 << sn) / (r["median_ms"] * 1e-3) / 1e9,
-                          "pass_ms": r["pass_ms"]})
+                          "gbs": gbs, "roofline_frac": gbs / peak,
+                          "slowest_pass_frac": 16.0 * (1 << sn) / (slow * 1e-3) / 1e9 / peak,
+                          "pass_ms": r["pass_ms"], "pass_kernels": kinds})
             r["plan"].close()
             del r
             torch.cuda.empty_cache()
 
     batched = []
-    if args.batched and rank == 0:
+    if args.batched and rank == 0 and world == 1:
         try:
             del state
         except Exception:  # already released by the sweep
@@ -412,21 +458,33 @@ def main():
             bn, bb = (int(v) for v in pair.split(":"))
             r = time_config(qft, torch, bn, None, args, 10, 3, per_pass=True, log2_batch=bb)
             tot = 1 << (bn + bb)
+            gbs = r["passes"] * 16.0 * tot / (r["median_ms"] * 1e-3) / 1e9
             batched.append({"n": bn, "log2_batch": bb, "passes": r["passes"], "median_ms": r["median_ms"],
                             "gflops": 5.0 * tot * bn / (r["median_ms"] * 1e-3) / 1e9,
-                            "gbs": r["passes"] * 16.0 * tot / (r["median_ms"] * 1e-3) / 1e9, "pass_ms": r["pass_ms"]})
+                            "gbs": gbs, "roofline_frac": gbs / peak, "pass_ms": r["pass_ms"]})
             r["plan"].close()
             del r
             torch.cuda.empty_cache()
 
-    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N = 1 only ----
+    # ---- CPU baseline: the oracle as it stands, WHOLE circuits, rank 0 at N = 1 only ----
+    # 1 warm-up + 3 trials, median, at n = 22 (to sit beside PAPER.md:185's 3.86 s / 0.064 s)
+    # and n = 26 (the largest size whose whole circuit takes seconds); a bounded sample of the n = 30 workload
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         try:
             torch.cuda.empty_cache()
-            est, spent, sdesc, cores = oracle_sample(n, args.k)
-            cpu_baseline = {"value": flops / est / 1e9, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
-                            "sample": sdesc, "seconds_estimated": est}
+            t22, cores = oracle_full(22, args.k)
+            t26, cores = oracle_full(26, args.k)
+            m22, m26 = sorted(t22)[1], sorted(t26)[1]
+            cpu_baseline = {"value": 5.0 * (1 << 26) * 26 / m26 / 1e9, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
+                            "sample": ("whole gate-by-gate oracle circuit (fp64, OpenMP), 1 warm-up + 3 trials, median, at "
+                                       f"n=26: {m26:.3f} s (value = 5 N log2 N / t there) and n=22: {m22:.4f} s; bounded "
+                                       f"sample of the n={n} workload: same circuit, smaller states"),
+                            "seconds_n26": m26, "seconds_n22": m22, "trials_n26": t26, "trials_n22": t22,
+                            "gflops_n22": 5.0 * (1 << 22) * 22 / m22 / 1e9}
+            if n >= 28 and args.extrapolate_cpu:
+                est, spent, sdesc, _ = oracle_sample(n, args.k)
+                cpu_baseline["extrapolated_not_measured"] = {"n": n, "seconds": est, "how": sdesc}
         except Exception as exc:
             cpu_baseline = {"value": None, "unit": "GFLOP/s", "cores": os.cpu_count(), "kind": "oracle",
                             "sample": f"failed: {exc}"}
@@ -439,12 +497,12 @@ def main():
             "config": {"workload": workload_text(n, args.k),
                        "n_qubits": n, "aqft_cutoff_k": desc["k"], "passes": npass, "ideal_passes": math.ceil(n / 13),
                        "tile_bits": desc["tile_bits"], "hub_bits": desc["hub_bits"], "folded_bit_reversal": desc["folded"],
+                       "tensor_memory_extended_tile": desc["ext_tile"],
                        "l2": "state larger than L2, no flush needed" if 8 * N > 2 * 126e6 else
                              "state fits L2: HBM fraction not meaningful",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "time_ms": ms_per_step, "hbm_gbs": roofline["step_gbs"], "hbm_frac_of_measured_peak": roofline["step_frac"],
-            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline, "gpu_launches": steps * plan.num_launches
-            if not sweep else steps * npass,
+            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline, "gpu_launches": steps * npass,
             "clocks": clocks,
         }
         if sweep:

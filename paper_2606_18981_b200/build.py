@@ -32,15 +32,16 @@ def _stale() -> bool:
     return False
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every source to an object file in parallel (one nvcc process each), then link."""
-    if force or _stale():
+def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str = LIB) -> str:
+    """Compile every source to an object file in parallel (one nvcc process each), then link.
+    extra_flags / lib: a differently configured build beside the product's (e.g. -DQFT_PHASE_TIMING)."""
+    if force or _stale() or lib != LIB:
         from concurrent.futures import ThreadPoolExecutor
 
         nvcc = os.environ.get("NVCC", "nvcc")
-        objdir = os.path.join(HERE, "build")
+        objdir = os.path.join(HERE, "build" if lib == LIB else "build_" + os.path.basename(lib))
         os.makedirs(objdir, exist_ok=True)
-        cflags = [f for f in NVCC_FLAGS if f not in ("-shared",)]
+        cflags = [f for f in NVCC_FLAGS if f not in ("-shared",)] + list(extra_flags)
 
         def compile_one(src: str) -> str:
             obj = os.path.join(objdir, os.path.splitext(src)[0] + ".o")
@@ -51,8 +52,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
             objs = list(ex.map(compile_one, SOURCES))
         subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static",
-                        "-o", LIB] + objs, check=True)
-    return LIB
+                        "-o", lib] + objs, check=True)
+    return lib
 
 
 if __name__ == "__main__":

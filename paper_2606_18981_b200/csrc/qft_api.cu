@@ -200,4 +200,13 @@ const char* qft_status_string(qft_status_t status) {
 
 const char* qft_last_cuda_error(void) { return g_cuda_err.c_str(); }
 
+#ifdef QFT_PHASE_TIMING
+// profiling builds only: device buffer of 16 counters the TMA kernel of pass `pass_index` accumulates into
+int qft_debug_set_phase_buffer(qft_plan_t plan, int pass_index, void* device_counters) {
+    if (!plan || pass_index < 0 || pass_index >= (int)plan->host.passes.size()) return 1;
+    plan->host.passes[pass_index].dbg = (unsigned long long*)device_counters;
+    return 0;
+}
+#endif
+
 }  // extern "C"

@@ -218,12 +218,24 @@ static int sm_count(int dev) {
     return v;
 }
 
+// The opt-in ceiling of dynamic shared memory on this device.  Every kernel gets this value as its attribute
+// (it only lifts the 48 KB default; occupancy follows the bytes a launch actually asks for), so passes that
+// share one kernel function but need different table sizes cannot lower each other's limit.
+static int smem_optin(int dev) {
+    static int cached[64] = {0};
+    if (dev < 0 || dev >= 64) return 227 * 1024;
+    if (cached[dev] > 0) return cached[dev];
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess || v <= 0) return 227 * 1024;
+    cached[dev] = v;
+    return v;
+}
+
 static cudaError_t launch_plain(const QftPassDesc& d, QftPassCache* cache, int dev, void* state, cudaStream_t stream) {
     pass_kernel_t kern = pick_kernel(d);
     const size_t smem = (size_t)8 << d.f;
     if (smem > 48 * 1024 && cache->attr_dev != dev) {
-        cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             8 << QFT_MAX_TILE_BITS);
+        cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin(dev));
         if (e != cudaSuccess) return e;
         cache->attr_dev = dev;
     }
@@ -268,7 +280,7 @@ static bool encode_map(const QftPassDesc& d, void* state, CUtensorMap* map) {
 static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int dev, void* state, cudaStream_t stream) {
     tma2_kernel_t kern = pick_tma2(d);
     if (!kern) return cudaErrorNotSupported;
-    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb);
+    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb, d.ntile);
     CUtensorMap map;
     {
         std::lock_guard<std::mutex> lock(cache->mu);
@@ -295,7 +307,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int de
             e.map = map;
         }
         if (cache->attr_dev != dev) {
-            cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaError_t e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin(dev));
             if (e != cudaSuccess) return e;
             cache->attr_dev = dev;
         }

@@ -154,6 +154,47 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) 
     return true;
 }
 
+// Deferred swaps (QFT_FLAG_DEFER_SWAPS; "SWAP can be deferred to I/O or absorbed into layout",
+// :137 "the final swaps are not implemented as gates but accounted for in the caller as an output index
+// permutation"): the planner no longer steers towards the bit-reversed layout, it takes the cheapest one and the
+// plan reports where every qubit ended (QftHostPlan::out_qubit_at).  K = ceil(n / w) passes, no pair passes at
+// all: the hub's qubits trade places with the top l qubits in the first pass (a qubit cannot be processed while
+// it sits on a hub bit) and are processed up there by the last pass; every other window is processed where it
+// sits.  Final layout: the circuit's own (qubit q on bit q) except that bits a and n-1-a are exchanged for a < l.
+bool build_deferred(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) {
+    if (n <= fmax) return false;
+    const int w = std::min(wcap, fmax - l);
+    if (w < l || w < 1) return false;
+    const int K = ilog2_ceil_div(n, w);
+    if (K < 2) return false;
+    std::vector<int> sizes = split_balanced(n, K);
+    if (sizes.back() < l || sizes.front() < l) return false;
+    const int f = fmax;
+    int t = n - 1;
+    for (int p = 0; p < K; ++p) {
+        PassSpec ps;
+        for (int i = 0; i < sizes[p]; ++i) ps.window.push_back(t - i);
+        const int lo = t - sizes[p] + 1;
+        std::set<int> F;
+        for (int a = 0; a < l; ++a) F.insert(a);
+        if (p == K - 1) {
+            // qubits lo .. l sit on their own addresses, qubits l-1 .. 0 on the top l addresses (reversed)
+            for (int a = l; a <= t; ++a) F.insert(a);
+            for (int a = n - l; a < n; ++a) F.insert(a);
+        } else {
+            for (int a = lo; a <= t; ++a) F.insert(a);
+        }
+        ps.F.assign(F.begin(), F.end());
+        if (p == 0)
+            for (int a = 0; a < l; ++a) { ps.moves.push_back({a, n - 1 - a}); ps.moves.push_back({n - 1 - a, a}); }
+        if (p > 0 && p < K - 1) ps.extras_above = t;
+        add_extras(ps, n, f);
+        t -= sizes[p];
+        out->push_back(ps);
+    }
+    return true;
+}
+
 std::vector<int> step_sizes(int w, bool force2 = false) {
     if (w <= 0) return {};
     if (force2 && w >= 2 && w <= 5) return split_balanced(w, 2);  // two register groups for the TMA kernel
@@ -624,6 +665,7 @@ static bool lower_all(const QftPlanParams& prm, std::vector<PassSpec>& specs, in
         out->passes.push_back(d);
     }
     out->window = wmaxseen;
+    out->out_qubit_at = qubit_at;
     return true;
 }
 
@@ -639,12 +681,18 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         *err = "invalid argument";
         return 1;
     }
-    if (prm.flags & ~(1u | 2u | 4u | 16u)) { *err = "unknown flag"; return 2; }
+    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u)) { *err = "unknown flag"; return 2; }
+    if ((prm.flags & 32u) && (prm.flags & 2u)) { *err = "deferred swaps have no unfolded schedule"; return 2; }
     // defaults from the B200 sweeps (profiles/r01_tile_hub_sweep.md, profiles/r02_tile_hub_sweep.md): 128-byte
     // granules (hub 4) as soon as the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit
     // windows pay off (n = 13: three multi-CTA passes on 2^12 tiles take 17 us, one 8192-amplitude CTA takes 30 us)
     int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : (n == 13 && prm.batch_bits == 0 ? 12 : 13));
+    // 256-byte granules (hub 5) where a 10-qubit window still gives the minimum number of passes: with the
+    // tensor-memory extension that is n = 26 ... 30 (3 passes) and n = 34 (4 passes); n = 31 ... 33 need 11-qubit
+    // windows for 3 passes, i.e. 128-byte granules (profiles/r02_tile_hub_sweep.md)
     int l = prm.hub_bits ? prm.hub_bits : (na >= 20 ? 4 : 3);
+    if (!prm.hub_bits && prm.batch_bits == 0 && fmax == 14 && !(prm.flags & (1u | 2u | 4u | 16u)) && ((n >= 26 && n <= 30) || n == 34))
+        l = 5;
     if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 6 || l >= fmax) {
         *err = "unsupported tile_bits / hub_bits";
         return 2;
@@ -663,15 +711,29 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     out->n_swap = n / 2;
 
     // tensor-memory extended tiles (one more window qubit per pass than the shared-memory tile holds): only for
-    // 2^14 tiles, single transforms, TMA kernels allowed; tried first, dropped if any pass cannot be lowered
+    // 2^14 tiles (two CTAs per SM on 2^13 halves measured slower: profiles/r02_ext_tile.md), single transforms, TMA
+    // kernels allowed; tried first, dropped if any pass cannot be lowered
     const bool ext_ok = fmax == 14 && prm.batch_bits == 0 && !(prm.flags & (1u | 2u | 4u | 16u)) && n > fmax + 1;
+    if ((prm.flags & 32u) && prm.batch_bits != 0) { *err = "deferred swaps are not available for batched plans"; return 2; }
     for (int attempt = ext_ok ? 0 : 1; attempt < 2; ++attempt) {
         const int fplan = attempt == 0 ? fmax + 1 : fmax;  // tile bits the schedule may use
         std::vector<PassSpec> specs;
         out->passes.clear();
         out->ext_tile = attempt == 0;
         out->folded = false;
-        if (!(prm.flags & 2u)) out->folded = build_folded(n, prm.max_fused, fplan, l, &specs);
+        if (prm.flags & 32u) {
+            if (n <= fmax) {
+                build_unfolded(n, prm.max_fused, fmax, l, &specs);  // one tile: simply leave the reversal out
+                specs.back().moves.clear();
+            } else if (!build_deferred(n, prm.max_fused, fplan, l, &specs)) {
+                if (attempt == 0) continue;
+                *err = "deferred swaps: windows smaller than the hub cannot be scheduled";
+                return 2;
+            }
+            out->folded = true;  // no stand-alone permutation pass
+        } else if (!(prm.flags & 2u)) {
+            out->folded = build_folded(n, prm.max_fused, fplan, l, &specs);
+        }
         if (!out->folded) {
             if (attempt == 0) continue;  // the extension only exists for folded schedules
             specs.clear();
@@ -959,8 +1021,12 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
         ++pi;
     }
     if (next_qubit != -1) { *err = "self-check: not every qubit was processed"; return 5; }
-    for (int a = 0; a < n; ++a)
-        if (qubit_at[a] != (a < nq ? nq - 1 - a : a)) { *err = "self-check: final layout is not the bit reversal"; return 5; }
+    const bool deferred = (plan.prm.flags & 32u) != 0;  // swaps left to the caller: any layout, but the reported one
+    if ((int)plan.out_qubit_at.size() != n) { *err = "self-check: output layout missing"; return 5; }
+    for (int a = 0; a < n; ++a) {
+        if (qubit_at[a] != plan.out_qubit_at[a]) { *err = "self-check: final layout differs from the reported one"; return 5; }
+        if (!deferred && qubit_at[a] != (a < nq ? nq - 1 - a : a)) { *err = "self-check: final layout is not the bit reversal"; return 5; }
+    }
     const bool want_scale = plan.prm.norm != 1;
     if ((want_scale && nscaled != 1) || (!want_scale && nscaled != 0)) { *err = "self-check: scale"; return 5; }
     return 0;
@@ -995,9 +1061,12 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
     o << "{\"n\":" << plan.prm.n << ",\"batch_bits\":" << plan.prm.batch_bits << ",\"k\":" << plan.k_eff << ",\"sign\":" << plan.prm.sign
       << ",\"norm\":" << plan.prm.norm << ",\"max_fused_qubits\":" << plan.prm.max_fused
       << ",\"tile_bits\":" << plan.tile_bits << ",\"hub_bits\":" << plan.hub_bits
-      << ",\"folded\":" << (plan.folded ? "true" : "false") << ",\"ext_tile\":" << (plan.ext_tile ? "true" : "false")
+      << ",\"folded\":" << (plan.folded ? "true" : "false") << ",\"swaps\":\"" << ((plan.prm.flags & 32u) ? "deferred" : "applied")
+      << "\",\"ext_tile\":" << (plan.ext_tile ? "true" : "false")
       << ",\"n_h\":" << plan.n_h << ",\"n_cr\":" << plan.n_cr
-      << ",\"n_swap\":" << plan.n_swap << ",\"passes\":[";
+      << ",\"n_swap\":" << plan.n_swap << ",\"out_qubit_of_bit\":[";
+    for (size_t a = 0; a < plan.out_qubit_at.size(); ++a) o << (a ? "," : "") << plan.out_qubit_at[a];
+    o << "],\"passes\":[";
     for (size_t i = 0; i < plan.passes.size(); ++i) {
         const QftPassDesc& d = plan.passes[i];
         if (i) o << ",";

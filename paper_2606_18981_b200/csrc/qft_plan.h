@@ -26,7 +26,8 @@
 // 5 coords + the tensor-memory base address
 #define QFT_TMA2_MID_STRIDE 9   // float2 per row (<= 5 used; odd: rows of different lanes fall into different banks)
 #define QFT_TMA2_END_STRIDE 17  // float2 per row (R1 + R2 + 1 <= 11 used; odd for the same reason)
-#define QFT_TMA2_TABLE_BYTES(eb) ((32 * QFT_TMA2_MID_STRIDE + 2 * ((eb) > 5 ? (1 << (eb)) : 32) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24)
+#define QFT_TMA2_TABLE_BYTES(eb, ntile) \
+    ((32 * QFT_TMA2_MID_STRIDE + 2 * ((eb) > 5 ? (1 << (eb)) : 32) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24 + (((ntile) + 7) >> 3) * 256 * 16)
 
 struct QftStep {
     int8_t r;     // qubits in the group
@@ -102,6 +103,9 @@ struct QftPassDesc {
     int8_t t2_addr[16], t2_canon[16], r2_addr[QFT_MAX_RADIX_BITS + 3];
     uint8_t swz_col[16];
     QftTma2Desc tma;
+#ifdef QFT_PHASE_TIMING
+    unsigned long long* dbg;  // profiling builds only: 16 counters, clocks per phase of CTA 0 (qft_tma.cuh)
+#endif
 };
 
 #include <string>
@@ -126,6 +130,7 @@ struct QftHostPlan {
     bool folded = false;
     bool ext_tile = false;  // some passes use the tensor-memory extended tile
     std::vector<QftPassDesc> passes;
+    std::vector<int> out_qubit_at;  // after the last pass address bit a holds logical qubit out_qubit_at[a]
     long long n_h = 0, n_cr = 0, n_swap = 0;
 };
 

@@ -164,6 +164,18 @@ struct BatchApply {
     }
 };
 
+// Profiling builds (-DQFT_PHASE_TIMING): thread 0 of CTA 0 accumulates the clocks between phase boundaries.
+#ifdef QFT_PHASE_TIMING
+#define QFT_PHASE(i)                                                       \
+    if (d.dbg && blockIdx.x == 0 && tid == 0) {                            \
+        const long long now_ = clock64();                                  \
+        atomicAdd(d.dbg + (i), (unsigned long long)(now_ - tlast_));       \
+        tlast_ = now_;                                                     \
+    }
+#else
+#define QFT_PHASE(i)
+#endif
+
 template <int R1, int R2, int KC, int LT, int XT>
 __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     qft_pass_tma2(float2* __restrict__ state, const __grid_constant__ CUtensorMap tmap,
@@ -178,6 +190,11 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     float2* endW = reinterpret_cast<float2*>(nextc + 6);     // two end tables (by parity) of max(32, 2^eb) rows
     const uint32_t tid = threadIdx.x;
     const QftTma2Desc& t = d.tma;
+    const uint32_t end_rows = t.eb > 5 ? (1u << t.eb) : 32u;
+    // tile-index byte -> address bits (tblA) and logical qubit bits (tblL): 256 entries per byte of the tile index
+    const int nslice = (d.ntile + 7) >> 3;
+    uint64_t* tblA = reinterpret_cast<uint64_t*>(endW + 2 * end_rows * kEndStride);
+    uint64_t* tblL = tblA + nslice * 256;
 
     // ---- per-thread constants ----
     uint32_t off1_ld = xor_cols(t.s1_tid_ld, tid, LT);
@@ -198,7 +215,20 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     }
     const int k = d.k;
     const int win_lo = d.win_lo;
-    const uint64_t lbmask = (win_lo > 0) ? ((1ull << win_lo) - 1ull) : 0ull;
+    // this thread's entry of the per-tile end table (see the tile walk): row e, column q, target qubit, the bits
+    // below it that may hold controls, and the phase its own row bits e contribute
+    const uint32_t end_cnt = (uint32_t)NQ << t.eb;
+    const uint32_t end_e = tid / NQ, end_q = tid % NQ;
+    const uint32_t end_slot = end_e * kEndStride + end_q;
+    const int end_tq = (XT && end_q == (uint32_t)(R1 + R2)) ? win_lo - 1 : win_lo + (int)end_q;
+    const uint64_t end_mask = (1ull << (end_tq < win_lo ? (end_tq > 0 ? end_tq : 0) : (win_lo > 0 ? win_lo : 0))) - 1ull;
+    uint32_t end_ph_e;
+    {
+        uint64_t Le = 0;
+        for (int b = 0; b < t.eb; ++b)
+            if ((end_e >> b) & 1u) Le |= 1ull << t.e_log[b];
+        end_ph_e = qftp::cr_phase_u32(Le & end_mask, end_tq > 0 ? end_tq : 0, k);
+    }
 
     // let the next pass's CTAs be scheduled as soon as SM resources free up (they wait below)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -223,6 +253,18 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
             if ((u1 >> q) & 1u) ph += qftp::cr_phase_u32(1ull << (t.t2_lo + (int)b), t.t1_lo + q, k);
         midW[u1 * kMidStride + b] = qftp::cis_fwd_u32(ph);
     }
+    for (int i = (int)tid; i < nslice * 256; i += NT) {
+        uint64_t a = 0, L = 0;
+        for (int b = 0; b < 8; ++b) {
+            const int bit = (i >> 8) * 8 + b;
+            if (bit < d.ntile && ((i >> b) & 1)) {
+                a |= 1ull << d.tile_addr[bit];
+                L |= 1ull << d.log_tile[bit];
+            }
+        }
+        tblA[i] = a;
+        tblL[i] = L;
+    }
     __syncthreads();
     if constexpr (XT) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -237,80 +279,85 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     const uint32_t nunits = (1u << nbig) / csz;
     const uint32_t ustride = gridDim.x / csz;
     const bool has_end = win_lo > 0;
-    const uint32_t end_rows = t.eb > 5 ? (1u << t.eb) : 32u;
 
-    // tile index (+ half) -> TMA coordinates (HBM address bits of the tile, cut into the tensor map's dims)
-    auto coords_of = [&](uint32_t un, uint32_t half, int (&c)[5]) {
+    // tile index (+ half) -> HBM base address / logical bits, one table lookup per index byte
+    auto lut = [&](const uint64_t* T, uint32_t m) {
+        uint64_t r = T[m & 255u];
+        if (nslice > 1) r |= T[256 + ((m >> 8) & 255u)];
+        if (nslice > 2) r |= T[512 + ((m >> 16) & 255u)];
+        if (nslice > 3) r |= T[768 + (m >> 24)];
+        return r;
+    };
+    // lanes 0-4 of warp 0 each own one TMA coordinate: the tile's address bits cut into the tensor map's dims
+    const int cj = tid < 5u ? (int)tid : 0;
+    const int c_lo = t.tma_lo[cj];
+    const uint64_t c_mask = (1ull << t.tma_len[cj]) - 1ull;
+    auto put_coords = [&](uint32_t un, uint32_t half) {
         uint32_t ml, ms;
         decode_tile(un * csz + rho, d.npair, &ml, &ms);
-        ml |= half << nbig;
-        uint64_t base = 0;
-        for (int i = 0; i < d.ntile; ++i)
-            if ((ml >> i) & 1u) base |= 1ull << d.tile_addr[i];
-#pragma unroll
-        for (int j = 0; j < 5; ++j) c[j] = (int)((base >> t.tma_lo[j]) & ((1ull << t.tma_len[j]) - 1ull));
+        nextc[tid] = (int)((lut(tblA, ml | (half << nbig)) >> c_lo) & c_mask);
     };
 
     // everything above is independent of the state; the previous pass must have completed (and its
     // writes be visible) before the first load
     asm volatile("griddepcontrol.wait;" ::: "memory");
     uint32_t unit = blockIdx.x / csz;
-    if (unit < nunits && tid == 0) {
-        int c[5];
-        coords_of(unit, 0u, c);
-        mbar_expect_tx(mbar, 8u << F);
-        tma_load_5d(smem_raw, &tmap, mbar, c[0], c[1], c[2], c[3], c[4]);
+    if (unit < nunits && tid < 32u) {
+        if (tid < 5u) put_coords(unit, 0u);
+        __syncwarp();
+        if (tid == 0) {
+            mbar_expect_tx(mbar, 8u << F);
+            tma_load_5d(smem_raw, &tmap, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
+        }
+        __syncwarp();
     }
     uint32_t parity = 0;
+#ifdef QFT_PHASE_TIMING
+    long long tlast_ = clock64();
+#endif
     for (; unit < nunits; unit += ustride) {
 #pragma unroll 1
         for (uint32_t half = 0; half <= (uint32_t)XT; ++half) {
         // ---- bookkeeping while the tile's load is in flight (few registers live here) ----
         const bool last_half = half == (uint32_t)XT;
         const bool has_next = !last_half || unit + ustride < nunits;
-        uint64_t base_st = 0;
+        uint64_t base_st;
         float2* endWp = endW + parity * (end_rows * kEndStride);
         {
             uint32_t ml, ms;
             decode_tile(unit * csz + rho, d.npair, &ml, &ms);
-            ml |= half << nbig;
-            uint64_t Ltile = 0;
-            for (int i = 0; i < d.ntile; ++i)
-                if ((ml >> i) & 1u) Ltile |= 1ull << d.log_tile[i];
-            for (int i = 0; i < nbig; ++i)
-                if ((ms >> i) & 1u) base_st |= 1ull << d.tile_addr[i];
+            const uint64_t Ltile = lut(tblL, ml | (half << nbig));
+            base_st = lut(tblA, ms);
             if (has_end) {
-                // end bases of this tile: endW[e][q] = product of the controlled-R_m from every qubit
-                // below the window (tile-index bits + in-tile bits e) onto the window's q-th qubit; with
-                // an extended tile the last column belongs to the extension's qubit win_lo - 1
-                const uint32_t cnt = (uint32_t)NQ << t.eb;
-                for (uint32_t i = tid; i < cnt; i += NT) {
+                // end bases of this tile: endW[e][q] = product of the controlled-R_m from every qubit below the
+                // window (tile-index bits + in-tile bits e) onto the window's q-th qubit (with an extended tile
+                // the last column belongs to the extension's qubit win_lo - 1).  The phase is linear over disjoint
+                // bit sets, so a thread's entry is its constant part from e plus the tile's part.
+                if (tid < end_cnt)
+                    endWp[end_slot] = qftp::cis_fwd_u32(end_ph_e + qftp::cr_phase_u32(Ltile & end_mask, end_tq, k));
+                for (uint32_t i = tid + NT; i < end_cnt; i += NT) {  // only when 2^eb (R1 + R2 + XT) > threads
                     const uint32_t e = i / NQ, q = i % NQ;
                     uint64_t L = Ltile;
                     for (int b = 0; b < t.eb; ++b)
                         if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
-                    L &= lbmask;
                     int tq = win_lo + (int)q;
-                    if (XT && q == (uint32_t)(R1 + R2)) {
-                        tq = win_lo - 1;
-                        L &= (1ull << tq) - 1ull;
-                    }
+                    if (XT && q == (uint32_t)(R1 + R2)) tq = win_lo - 1;
+                    L &= (1ull << (tq < win_lo ? tq : win_lo)) - 1ull;
                     endWp[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, tq, k));
                 }
             }
-            if (tid == 0 && has_next) {
-                int c[5];
-                if (last_half) coords_of(unit + ustride, 0u, c);
-                else coords_of(unit, half + 1u, c);
-#pragma unroll
-                for (int j = 0; j < 5; ++j) nextc[j] = c[j];
+            if (tid < 5u && has_next) {
+                if (last_half) put_coords(unit + ustride, 0u);
+                else put_coords(unit, half + 1u);
             }
         }
         float2 x[32];
         // keep the 96 per-register shared-memory offsets out of loop-invariant hoisting (they would
         // spill): one XOR next to each access is cheaper than a local-memory reload
         asm volatile("" : "+r"(off1_ld), "+r"(off1_mid), "+r"(off2_mid));
+        QFT_PHASE(0)
         mbar_wait(mbar, parity);
+        QFT_PHASE(1)
         // this CTA's whole tile is on chip (or in registers / tensor memory): the partner may overwrite it in HBM
         if (d.npair && last_half) cluster_arrive_relaxed();
 
@@ -322,6 +369,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         QFT_ALL32(QFT_LD1)
 #undef QFT_LD1
         __syncthreads();  // every amplitude of the tile is in a register: the buffer becomes the exchange
+        QFT_PHASE(2)
         if (d.conj) {
 #pragma unroll
             for (int B = 0; B < 32; ++B) x[B].y = -x[B].y;
@@ -331,6 +379,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         QFT_ALL32(QFT_ST1)
 #undef QFT_ST1
         __syncthreads();
+        QFT_PHASE(3)
 
         // ------------------------------ step 2 ------------------------------
 #define QFT_LD2(B) x[B] = lds64(smem_raw, off2_mid ^ reg_off<B>(c2mid));
@@ -343,6 +392,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
             mbar_expect_tx(mbar, 8u << F);
             tma_load_5d(smem_raw, &tmap, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
         }
+        QFT_PHASE(4)
 
         {
             // the phases group 2's qubits put on group 1's frequency bits, applied here, after
@@ -391,6 +441,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
 #pragma unroll
             for (int B = 0; B < 32; ++B) x[B] = qftp::cscale(x[B], d.scale);
         }
+        QFT_PHASE(5)
         if constexpr (XT) {
             if (!last_half) {
                 // first half: park the results in tensor memory until the second half has caught up
@@ -398,6 +449,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
                 tmem_park16<16>(tpark + 32u, x);
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 parity ^= 1u;
+                QFT_PHASE(6)
                 continue;
             }
         }
@@ -451,6 +503,10 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
             }
         }
         parity ^= 1u;
+        QFT_PHASE(7)
+#ifdef QFT_PHASE_TIMING
+        if (d.dbg && blockIdx.x == 0 && tid == 0) atomicAdd(d.dbg + 8, 1ull);
+#endif
         }
     }
 #undef QFT_ALL32

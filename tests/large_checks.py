@@ -123,18 +123,28 @@ def tones_closed_form_chunk(n: int, k: int, freqs, phases, K: torch.Tensor) -> t
     return acc
 
 
-def tones_rel_l2(y: torch.Tensor, n: int, k: int, freqs, phases, chunk_bits: int = 22, index_chunks=None):
-    """Relative L2 distance between the device result y and the closed form, over all outputs or
-    over the listed chunks of 2^chunk_bits consecutive outputs.  Returns (rel_l2, ref_norm2)."""
+def tones_parity(y: torch.Tensor, n: int, k: int, freqs, phases, chunk_bits: int = 22, index_chunks=None):
+    """Distance between the device result y and the closed form, over all outputs or over the listed chunks of
+    2^chunk_bits consecutive outputs: (relative L2, sum |ref|^2, max |y - ref|, max |ref|)."""
     cb, C, nc = _chunks(n, chunk_bits)
     dev = y.device
     base = torch.arange(C, dtype=torch.int64, device=dev)
     num = torch.zeros((), dtype=torch.float64, device=dev)
     den = torch.zeros((), dtype=torch.float64, device=dev)
+    mx = torch.zeros((), dtype=torch.float64, device=dev)
+    rmax = torch.zeros((), dtype=torch.float64, device=dev)
     for c in (range(nc) if index_chunks is None else index_chunks):
         K = base + c * C
         ref = tones_closed_form_chunk(n, k, freqs, phases, K)
         d = y[c * C:(c + 1) * C].to(torch.complex128) - ref
         num += (d.real * d.real + d.imag * d.imag).sum()
         den += (ref.real * ref.real + ref.imag * ref.imag).sum()
-    return math.sqrt(float(num.item()) / float(den.item())), float(den.item())
+        mx = torch.maximum(mx, d.abs().max())
+        rmax = torch.maximum(rmax, ref.abs().max())
+    return math.sqrt(float(num.item()) / float(den.item())), float(den.item()), float(mx.item()), float(rmax.item())
+
+
+def tones_rel_l2(y: torch.Tensor, n: int, k: int, freqs, phases, chunk_bits: int = 22, index_chunks=None):
+    """(relative L2, sum |ref|^2) of tones_parity."""
+    rel, den, _, _ = tones_parity(y, n, k, freqs, phases, chunk_bits, index_chunks)
+    return rel, den

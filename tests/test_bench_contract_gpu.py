@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 def test_bench_line_has_the_contract_keys():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--n", "22", "--steps", "5", "--warmup", "3",
-                        "--batched", "10:12"], capture_output=True, text=True, timeout=600)
+                        "--batched", "10:12", "--sweep", "24"], capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [ln for ln in r.stdout.splitlines() if ln.strip()]
     assert len(lines) == 1
@@ -34,3 +34,7 @@ def test_bench_line_has_the_contract_keys():
     assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] > 0 and cb["sample"]
     assert d["gpu_launches"] == 5 * d["config"]["passes"]
     assert d["batched"][0]["n"] == 10 and d["batched"][0]["log2_batch"] == 12
+    sw = d["sweep"][0]
+    assert sw["n"] == 24 and sw["passes"] >= sw["ideal_passes"] and 0 < sw["roofline_frac"] < 1.2
+    assert "seconds_n22" in cb and "seconds_n26" in cb and len(cb["trials_n26"]) == 3  # whole circuits, timed
+    assert rf["traffic"] is None or rf["traffic_source"]

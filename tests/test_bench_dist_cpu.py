@@ -67,3 +67,17 @@ def test_reference_arm_runs_on_rank_0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_reference_arm_times_whole_oracle_circuits():
+    """bench.py --impl reference: every step is one whole oracle circuit (here n = 20: seconds on any host)."""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--n", "20", "--steps", "2",
+                        "--warmup", "1"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["steps"] == 2 and d["warmup"] == 1 and d["metric"] == "dft_equiv_gflops"
+    assert d["config"]["sample_n_qubits"] == 20 and d["cpu_baseline"]["kind"] == "oracle"
+    assert abs(d["value"] - 5.0 * (1 << 20) * 20 / (d["ms_per_step"] * 1e-3) / 1e9) < 1e-6 * d["value"]
+    assert d["e2e"]["value"] == d["value"] and d["e2e"]["h2d_bytes_per_step"] == 0

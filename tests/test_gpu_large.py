@@ -1,9 +1,12 @@
 """GPU parity at BASELINE.json's full sizes (configs 3-5), in the launch configuration bench.py times.
 
 n = 26: element by element against the CPU oracle (1 GiB of fp64 state), for every max_fused_qubits of
-config 3.  n = 30 and n = 33: beyond the oracle's practical size, so (north_star) closed-form
-sparse-tone outputs, Parseval, and float64 direct sums at sampled output indices
+config 3.  n = 28 and n = 30 (Gaussian input): element by element against the full oracle as well, so that
+the kernel instantiations the headline bench times are compared densely (the oracle needs 4 / 16 GiB of host
+memory and one to three minutes).  n = 30 and n = 33 otherwise: beyond the oracle's practical size, so
+(north_star) closed-form sparse-tone outputs, Parseval, and float64 direct sums at 32 sampled output indices
 (tests/large_checks.py, pinned to the oracle on the CPU by tests/test_large_checks_cpu.py).
+Bounds: tests/parity_bounds.py (north_star's relative L2, a regression bound, a max-abs element bound).
 """
 import math
 
@@ -12,9 +15,11 @@ import pytest
 
 import qft_inputs as qi
 
+from parity_bounds import MAXABS_FRAC, REG_L2, TOL_LARGE, ChunkedParity
+
 pytestmark = pytest.mark.gpu
 
-TOL_LARGE = 1e-4  # north_star: relative L2 <= 1e-4 up to n = 33
+NSAMPLES = 32  # north_star: double-precision direct sums at 32 sampled output indices
 
 
 def _free_gib():
@@ -34,17 +39,17 @@ def test_config3_n26_window_sweep_against_oracle():
     n = 26
     x = qi.gaussian(n, 1)
     ref = torch.from_numpy(oracle.qft(x)).cuda()
-    refn = float(torch.linalg.vector_norm(ref).item())
     passes = []
     for w in (2, 4, 6, 10, 13):
         plan = qft.Plan(n, n, w)
         t = torch.from_numpy(x).cuda()
         plan.execute(t)
         torch.cuda.synchronize()
-        err = float(torch.linalg.vector_norm(t.to(torch.complex128) - ref).item()) / refn
+        cp = ChunkedParity()
+        cp.add(t, ref)
         passes.append(plan.num_passes)
         plan.close()
-        assert err <= TOL_LARGE, (w, err)
+        cp.check(n, ("max_fused_qubits", w))
         del t
     assert passes == sorted(passes, reverse=True) and passes[-1] == 3
     # AQFT at the same size, one cutoff
@@ -53,13 +58,13 @@ def test_config3_n26_window_sweep_against_oracle():
     t = torch.from_numpy(x).cuda()
     plan.execute(t)
     torch.cuda.synchronize()
-    err = float(torch.linalg.vector_norm(t.to(torch.complex128) - refk).item()) / float(
-        torch.linalg.vector_norm(refk).item())
     plan.close()
-    assert err <= TOL_LARGE
+    cp = ChunkedParity()
+    cp.add(t, refk)
+    cp.check(n, "k = 8")
 
 
-def _sample_indices(n, freqs, seed, count=32):
+def _sample_indices(n, freqs, seed, count=NSAMPLES):
     rng = np.random.default_rng(seed)
     Ks = [int(f) for f in freqs]
     while len(Ks) < count:
@@ -96,8 +101,8 @@ def test_config4_n30_aqft_sweep_tones_closed_form():
             chunks = None  # every output index
         else:  # the chunks around the tone bins (where the energy is) + 24 random chunks
             chunks = sorted(set(near) | {int(c) for c in rng.integers(0, nchunks, size=24)})
-        rel, den = lc.tones_rel_l2(y, n, k, fr, ph, chunk_bits=22, index_chunks=chunks)
-        assert rel <= TOL_LARGE, (k, rel)
+        rel, den, mx, rmax = lc.tones_parity(y, n, k, fr, ph, chunk_bits=22, index_chunks=chunks)
+        assert rel <= TOL_LARGE and rel <= REG_L2 and mx <= MAXABS_FRAC * rmax, (k, rel, mx, rmax)
         if chunks is None:
             assert abs(den - 1.0) < 1e-9
         if k == 30:  # exact: five bins of modulus 1/sqrt 5, nothing else
@@ -106,19 +111,31 @@ def test_config4_n30_aqft_sweep_tones_closed_form():
         del y
 
 
+def _check_samples(got, want, what):
+    """Sampled outputs against the double-precision direct sums: the three bounds of parity_bounds on the sample."""
+    import torch
+
+    d = got - want
+    rel = float(torch.linalg.vector_norm(d).item() / torch.linalg.vector_norm(want).item())
+    assert rel <= TOL_LARGE, (what, "north_star tolerance", rel)
+    assert rel <= REG_L2, (what, "regression bound", rel)
+    assert float(d.abs().max().item()) <= MAXABS_FRAC * float(want.abs().max().item()), (what, "element bound")
+
+
 def test_config4_n30_gaussian_parseval_and_sampled_sums():
     import torch
 
     import large_checks as lc
     import paper_2606_18981_b200 as qft
 
-    if _free_gib() < 14:
-        pytest.skip("needs 14 GiB of free device memory")
+    if _free_gib() < 18:
+        pytest.skip("needs 18 GiB of free device memory")
     n = 30
     x = qi.gaussian_device(n, 2, device="cuda")
     fr, _ = qi.tone_params(n, 3, 5)
-    for k, count in ((30, 32), (12, 6)):
-        Ks = _sample_indices(n, fr, 31, count)
+    Ks = _sample_indices(n, fr, 31)
+    assert len(Ks) == NSAMPLES
+    for k in (4, 8, 12, 16, 30):  # every cutoff of config 4
         want = lc.sampled_outputs(x, Ks, k)  # from the actual fp32 device input, BEFORE the transform
         y = x.clone()
         plan = qft.Plan(n, k)
@@ -128,9 +145,53 @@ def test_config4_n30_gaussian_parseval_and_sampled_sums():
         assert abs(lc.norm2(y) - 1.0) < 1e-4
         got = y[torch.as_tensor(Ks, device="cuda")].to(torch.complex128)
         # |out[K]| ~ 2^-15 for a unit-norm Gaussian state: compare relative to the samples' norm
-        rel = float(torch.linalg.vector_norm(got - want).item() / torch.linalg.vector_norm(want).item())
-        assert rel <= TOL_LARGE, (k, rel)
+        _check_samples(got, want, ("n = 30 Gaussian", k))
         del y
+
+
+def _host_gib():
+    try:
+        import psutil
+
+        return psutil.virtual_memory().available / 2 ** 30
+    except Exception:
+        return 0.0
+
+
+@pytest.mark.parametrize("n,k", [(28, 28), (28, 5), (30, 30)])
+def test_dense_full_oracle_at_the_bench_kernels(n, k):
+    """Every output element of a Gaussian input against the full CPU oracle at n = 28 and n = 30: the default
+    plans here are made of the same kernel instantiations bench.py times (the tensor-memory extended 5+4+1
+    passes), which the tone inputs (a handful of non-zero outputs) and 32 samples cannot check densely."""
+    import torch
+
+    import oracle
+    import paper_2606_18981_b200 as qft
+
+    need_host = 28 * (1 << n) / 2 ** 30 + 4  # fp64 oracle state + complex64 input + slack
+    if _host_gib() < need_host:
+        pytest.skip(f"needs {need_host:.0f} GiB of free host memory for the oracle")
+    if _free_gib() < 3 * 8 * (1 << n) / 2 ** 30:
+        pytest.skip("not enough free device memory")
+    x = qi.gaussian_device(n, 2, device="cuda")
+    xh = x.cpu().numpy()
+    plan = qft.Plan(n, k)
+    bench = qft.Plan(30, 30)  # the headline workload's plan: same kernel, same register steps
+    shapes = lambda p: {(q["kernel"], tuple(q["steps"])) for q in p.describe()["passes"]}
+    if n == 28:
+        assert shapes(bench) <= shapes(plan) | {("tma2x", (5, 4, 1))} and ("tma2x", (5, 4, 1)) in shapes(plan)
+    bench.close()
+    plan.execute(x)
+    torch.cuda.synchronize()
+    plan.close()
+    ref = oracle.qft(xh, k)  # gate by gate on the host, complex128
+    del xh
+    cp = ChunkedParity()
+    C = 1 << 24
+    for c in range((1 << n) // C):
+        cp.add(x[c * C:(c + 1) * C], torch.from_numpy(ref[c * C:(c + 1) * C]).cuda())
+    rel, mx = cp.check(n, (n, k))
+    print(f"dense parity n={n} k={k}: rel_l2={rel:.3e} max_abs/max_ref={mx:.3e}")
 
 
 def test_config5_n33_tones_exact_and_k16():
@@ -147,23 +208,22 @@ def test_config5_n33_tones_exact_and_k16():
     nchunks = 1 << (n - 22)
     rng = np.random.default_rng(33)
     near = sorted({int(f) >> 22 for f in fr})
-    for k, count in ((33, 32), (16, 3)):
+    for k in (33, 16):
         qi.multi_tone_device(n, fr, ph, device="cuda", out=x)
         assert abs(lc.norm2(x) - 1.0) < 1e-5
-        Ks = _sample_indices(n, fr, 34, count)
+        Ks = _sample_indices(n, fr, 34)
         want = lc.sampled_outputs(x, Ks, k)  # direct fp64 sums over the 2^33 inputs, before the transform
         plan = qft.Plan(n, k)
-        assert plan.num_passes == 4
+        assert plan.num_passes == 3  # ceil(33 / 11): 11-qubit windows through the tensor-memory extension
         plan.execute(x)  # in place: 64 GiB, no second copy
         torch.cuda.synchronize()
         plan.close()
         assert abs(lc.norm2(x) - 1.0) < 1e-4
         got = x[torch.as_tensor(Ks, device="cuda")].to(torch.complex128)
-        err = float(torch.linalg.vector_norm(got - want).item() / torch.linalg.vector_norm(want).item())
-        assert err <= TOL_LARGE, (k, err)
+        _check_samples(got, want, ("n = 33 tones", k))
         chunks = sorted(set(near) | {int(c) for c in rng.integers(0, nchunks, size=40)})
-        rel, _ = lc.tones_rel_l2(x, n, k, fr, ph, chunk_bits=22, index_chunks=chunks)
-        assert rel <= TOL_LARGE, (k, rel)
+        rel, _, mx, rmax = lc.tones_parity(x, n, k, fr, ph, chunk_bits=22, index_chunks=chunks)
+        assert rel <= TOL_LARGE and rel <= REG_L2 and mx <= MAXABS_FRAC * rmax, (k, rel, mx, rmax)
         if k == 33:
             g5 = x[torch.as_tensor(fr, device="cuda")].to(torch.complex128).cpu().numpy()
             assert np.max(np.abs(g5 - np.exp(1j * ph) / math.sqrt(5))) < 1e-4
@@ -184,7 +244,7 @@ def test_max_size_n34_tones_exact():
     x = torch.empty(1 << n, dtype=torch.complex64, device="cuda")
     qi.multi_tone_device(n, fr, ph, device="cuda", out=x)
     assert abs(lc.norm2(x) - 1.0) < 1e-5
-    Ks = _sample_indices(n, fr, 35, 8)
+    Ks = _sample_indices(n, fr, 35)
     want = lc.sampled_outputs(x, Ks, n)
     plan = qft.Plan(n, n)
     plan.self_check()
@@ -193,12 +253,11 @@ def test_max_size_n34_tones_exact():
     plan.close()
     assert abs(lc.norm2(x) - 1.0) < 1e-4
     got = x[torch.as_tensor(Ks, device="cuda")].to(torch.complex128)
-    err = float(torch.linalg.vector_norm(got - want).item() / torch.linalg.vector_norm(want).item())
-    assert err <= TOL_LARGE, err
+    _check_samples(got, want, "n = 34 tones")
     rng = np.random.default_rng(34)
     near = sorted({int(f) >> 22 for f in fr})
     chunks = sorted(set(near) | {int(c) for c in rng.integers(0, 1 << (n - 22), size=24)})
-    rel, _ = lc.tones_rel_l2(x, n, n, fr, ph, chunk_bits=22, index_chunks=chunks)
-    assert rel <= TOL_LARGE, rel
+    rel, _, mx, rmax = lc.tones_parity(x, n, n, fr, ph, chunk_bits=22, index_chunks=chunks)
+    assert rel <= TOL_LARGE and rel <= REG_L2 and mx <= MAXABS_FRAC * rmax, (rel, mx, rmax)
     g5 = x[torch.as_tensor(fr, device="cuda")].to(torch.complex128).cpu().numpy()
     assert np.max(np.abs(g5 - np.exp(1j * ph) / math.sqrt(5))) < 1e-4

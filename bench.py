@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--extrapolate-cpu", action="store_true",
                     help="also estimate the oracle's time at the bench n from a few gates (labelled as extrapolated)")
     ap.add_argument("--sweep", default="26,33", help="comma list of extra n to time briefly ('' = none)")
@@ -419,6 +420,42 @@ def main():
             e2e = {"value": None, "unit": "GFLOP/s", "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 8 * N,
                    "error": str(exc)}
 
+    # ---- the variants of SURVEY.md section 8 (f2) at the same n, briefly: swaps deferred (the paper's own timed mode,
+    # PAPER.md:137) and out-of-place execute; reported beside the headline, not part of it ----
+    variants = None
+    if rank == 0 and world == 1 and not args.no_variants:
+        try:
+            vsteps = max(3, min(steps, 5))
+
+            def timed(fn):
+                for _ in range(2):
+                    fn()
+                torch.cuda.synchronize()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(vsteps):
+                    fn()
+                b.record(stream)
+                torch.cuda.synchronize()
+                return a.elapsed_time(b) / vsteps
+
+            dplan = qft.Plan(n, n if args.k is None else args.k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
+                             args.hub_bits, args.flags | qft.QFT_FLAG_DEFER_SWAPS)
+            d_ms = timed(lambda: qft.qft_execute(dplan.handle, state.data_ptr(), sptr))
+            variants = {"steps": vsteps, "defer_swaps": {"ms": d_ms, "passes": dplan.num_passes,
+                                                         "gbs": dplan.num_passes * 16.0 * N / (d_ms * 1e-3) / 1e9,
+                                                         "roofline_frac": dplan.num_passes * 16.0 * N / (d_ms * 1e-3) / 1e9 / peak}}
+            dplan.close()
+            free, _ = torch.cuda.mem_get_info()
+            if 8 * N * 1.05 < free:
+                out = torch.empty_like(state)
+                o_ms = timed(lambda: qft.qft_execute_oop(plan.handle, state.data_ptr(), out.data_ptr(), sptr))
+                variants["out_of_place"] = {"ms": o_ms, "passes": npass, "gbs": npass * 16.0 * N / (o_ms * 1e-3) / 1e9,
+                                            "roofline_frac": npass * 16.0 * N / (o_ms * 1e-3) / 1e9 / peak}
+                del out
+        except Exception as exc:
+            variants = {"error": str(exc)}
+
     # ---- optional brief sweep over other n (reported, not the headline) ----
     sweep = []
     if args.sweep and rank == 0 and world == 1:
@@ -505,6 +542,8 @@ def main():
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline, "gpu_launches": steps * npass,
             "clocks": clocks,
         }
+        if variants:
+            line["variants"] = variants
         if sweep:
             line["sweep"] = sweep
         if batched:

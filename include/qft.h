@@ -112,6 +112,18 @@ qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_bat
 #define QFT_FLAG_UNFOLDED 2u      /* natural-order passes + one stand-alone bit-reversal pass */
 #define QFT_FLAG_NO_TMA 4u        /* do not use the TMA-staged pass kernels */
 #define QFT_FLAG_NO_EXT_TILE 16u  /* do not extend 2^14 tiles by one qubit through tensor memory */
+/*
+ * QFT_FLAG_DEFER_SWAPS -- the paper's own mode ("the final swaps are not implemented as gates but
+ * accounted for in the caller as an output index permutation", "deferred to I/O or absorbed into
+ * layout"): the swap network is left out, the planner takes the cheapest layout (no tile exchanges between
+ * CTAs at all) and the plan reports it: after qft_execute, address bit a of the state holds the circuit's qubit
+ * qubit_of_bit[a] (qft_plan_output_order).  The natural-order result is recovered by the caller as
+ *     natural[K] = state[J],   bit a of J = bit (n-1-q) of K  with  q = qubit_of_bit[a].
+ * Without the flag qubit_of_bit[a] = n-1-a (J = K).  The layout chosen today is the circuit's own
+ * (qubit_of_bit[a] = a, i.e. plain bit-reversed output) except that bits a and n-1-a are exchanged for a below
+ * the granule size; callers must read it from the plan, not assume it.  Not available for batched plans.
+ */
+#define QFT_FLAG_DEFER_SWAPS 32u
 qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                                    qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
 
@@ -133,6 +145,16 @@ qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutof
  * device has no tensor memory / TMA: the library is built for sm_100a only).
  */
 qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream);
+
+/*
+ * qft_execute_oop -- out of place: device_out receives the transform of device_in, which is left untouched
+ * (same layout, alignment and ownership rules as qft_execute for both; the two buffers must be identical --
+ * then this is qft_execute -- or disjoint, QFT_ERR_INVALID_ARG otherwise).  The first pass loads its tiles from
+ * device_in through its tensor map and stores them into device_out, the remaining passes run in place on
+ * device_out, so the bytes moved are those of qft_execute: no extra copy, no scratch.  (A plan whose first pass
+ * is not a TMA pass -- states of fewer than about 2^14 amplitudes -- copies first.)  Only enqueues.
+ */
+qft_status_t qft_execute_oop(qft_plan_t plan, const void* device_in, void* device_out, void* stream);
 
 /*
  * qft_execute_host -- the same transform for a state in HOST memory (pageable or
@@ -160,6 +182,9 @@ qft_status_t qft_plan_destroy(qft_plan_t plan);
 int qft_plan_num_passes(qft_plan_t plan);   /* -1 if plan is NULL */
 int qft_plan_num_launches(qft_plan_t plan); /* kernels one qft_execute enqueues; -1 if NULL */
 qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_cr, long long* n_swap);
+/* qubit_of_bit[a], a < n_qubits: the circuit's qubit whose (frequency) bit address bit a holds after qft_execute;
+ * n-1-a for every plan without QFT_FLAG_DEFER_SWAPS (see there). */
+qft_status_t qft_plan_output_order(qft_plan_t plan, int* qubit_of_bit);
 /* JSON text describing every pass: kernel, tile address bits, window, register steps, store permutation,
  * pairing, and the fused block's gates ("each descriptor records the participating qubits, the
  * contiguous subrange of original gates folded into the block"): n_h, n_cr and [gate_first, gate_last], indices

@@ -21,13 +21,13 @@ LIB_PATH = os.path.join(_HERE, "libqft.so")
 
 QFT_OK, QFT_ERR_INVALID_ARG, QFT_ERR_UNSUPPORTED, QFT_ERR_ALLOC, QFT_ERR_CUDA, QFT_ERR_INTERNAL = range(6)
 QFT_NORM_UNITARY, QFT_NORM_NONE, QFT_NORM_INV_N = 0, 1, 2
-QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_NO_EXT_TILE = 1, 2, 4, 16
+QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_NO_EXT_TILE, QFT_FLAG_DEFER_SWAPS = 1, 2, 4, 16, 32
 QFT_MAX_QUBITS = 34
 
 EXPORTS = [
     "qft_plan_create", "qft_plan_create_batched", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
     "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
-    "qft_plan_describe_length", "qft_num_qubits_for", "qft_encode_padded",
+    "qft_plan_describe_length", "qft_num_qubits_for", "qft_encode_padded", "qft_execute_oop", "qft_plan_output_order",
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
     "qft_norm_sq", "qft_encode", "qft_rescale", "qft_fidelity", "qft_leakage",
 ]
@@ -67,6 +67,10 @@ def load() -> ctypes.CDLL:
     L.qft_plan_create_tuned.restype = ci
     L.qft_execute.argtypes = [vp, vp, vp]
     L.qft_execute.restype = ci
+    L.qft_execute_oop.argtypes = [vp, vp, vp, vp]
+    L.qft_execute_oop.restype = ci
+    L.qft_plan_output_order.argtypes = [vp, ctypes.POINTER(ci)]
+    L.qft_plan_output_order.restype = ci
     L.qft_execute_pass.argtypes = [vp, ci, vp, vp]
     L.qft_execute_pass.restype = ci
     L.qft_execute_host.argtypes = [vp, vp, vp]
@@ -150,6 +154,20 @@ def qft_execute(plan: int, device_state_ptr: int, stream: int = 0) -> None:
     st = load().qft_execute(plan, device_state_ptr, stream)
     if st != QFT_OK:
         raise QftError(st, "qft_execute")
+
+
+def qft_execute_oop(plan: int, device_in_ptr: int, device_out_ptr: int, stream: int = 0) -> None:
+    st = load().qft_execute_oop(plan, device_in_ptr, device_out_ptr, stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_execute_oop")
+
+
+def qft_plan_output_order(plan: int, n_qubits: int):
+    arr = (ctypes.c_int * n_qubits)()
+    st = load().qft_plan_output_order(plan, arr)
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_output_order")
+    return list(arr)
 
 
 def qft_execute_pass(plan: int, pass_index: int, device_state_ptr: int, stream: int = 0) -> None:
@@ -256,6 +274,7 @@ class Plan:
         if aqft_cutoff_k is None:
             aqft_cutoff_k = n_qubits
         self.n = n_qubits + log2_batch  # address bits of the state this plan transforms
+        self.n_qubits = n_qubits
         if log2_batch:
             if tile_bits or hub_bits or flags:
                 raise ValueError("the tuning knobs are not available for batched plans")
@@ -275,6 +294,21 @@ class Plan:
         if stream is None:
             stream = torch.cuda.current_stream(state.device).cuda_stream
         qft_execute(self.handle, state.data_ptr(), stream)
+
+    def execute_oop(self, src, dst, stream: int | None = None) -> None:
+        """dst <- transform of src (both CUDA complex64 tensors of 2^n elements); src is left untouched."""
+        import torch
+
+        for t in (src, dst):
+            if t.dtype != torch.complex64 or not t.is_cuda or not t.is_contiguous() or t.numel() != (1 << self.n):
+                raise ValueError("src and dst must be contiguous CUDA complex64 tensors of 2^n elements")
+        if stream is None:
+            stream = torch.cuda.current_stream(dst.device).cuda_stream
+        qft_execute_oop(self.handle, src.data_ptr(), dst.data_ptr(), stream)
+
+    def output_order(self):
+        """qubit_of_bit[a] for a < n_qubits (n-1-a unless the plan defers the swaps)."""
+        return qft_plan_output_order(self.handle, self.n_qubits)
 
     def execute_host(self, state, stream: int = 0) -> None:
         """state: numpy complex64 array or CPU torch tensor of 2^n elements; in place, synchronous."""

@@ -89,9 +89,39 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream) {
     const uintptr_t align = plan->host.prm.n >= 1 ? 16 : 8;
     if (((uintptr_t)device_state) & (align - 1)) return QFT_ERR_INVALID_ARG;
     for (size_t i = 0; i < plan->host.passes.size(); ++i) {
-        cudaError_t e = qft_launch_pass(plan->host.passes[i], &plan->cache[i], device_state, (cudaStream_t)stream);
+        cudaError_t e = qft_launch_pass(plan->host.passes[i], &plan->cache[i], device_state, device_state, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(e);
     }
+    return QFT_OK;
+}
+
+qft_status_t qft_execute_oop(qft_plan_t plan, const void* device_in, void* device_out, void* stream) {
+    if (!plan || !device_in || !device_out) return QFT_ERR_INVALID_ARG;
+    if ((((uintptr_t)device_in) | ((uintptr_t)device_out)) & 15) return QFT_ERR_INVALID_ARG;
+    if (device_in == device_out) return qft_execute(plan, device_out, stream);
+    const size_t bytes = (size_t)8 << (plan->host.prm.n + plan->host.prm.batch_bits);
+    const char *a = (const char*)device_in, *b = (const char*)device_out;
+    if ((a < b && a + bytes > b) || (b < a && b + bytes > a)) return QFT_ERR_INVALID_ARG;  // partial overlap
+    size_t first = 0;
+    if (!plan->host.passes.empty() && qft_pass_reads_through_tensor_map(plan->host.passes[0])) {
+        // the first pass reads its tiles from the input through the tensor map and stores them into the output
+        cudaError_t e = qft_launch_pass(plan->host.passes[0], &plan->cache[0], (void*)device_in, device_out, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(e);
+        first = 1;
+    } else {
+        cudaError_t e = cudaMemcpyAsync(device_out, device_in, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    for (size_t i = first; i < plan->host.passes.size(); ++i) {
+        cudaError_t e = qft_launch_pass(plan->host.passes[i], &plan->cache[i], device_out, device_out, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    return QFT_OK;
+}
+
+qft_status_t qft_plan_output_order(qft_plan_t plan, int* qubit_of_bit) {
+    if (!plan || !qubit_of_bit) return QFT_ERR_INVALID_ARG;
+    for (int a = 0; a < plan->host.prm.n; ++a) qubit_of_bit[a] = plan->host.out_qubit_at[a];
     return QFT_OK;
 }
 
@@ -99,7 +129,7 @@ qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_stat
     if (!plan || !device_state || pass_index < 0 || pass_index >= (int)plan->host.passes.size())
         return QFT_ERR_INVALID_ARG;
     if (((uintptr_t)device_state) & 15) return QFT_ERR_INVALID_ARG;
-    cudaError_t e = qft_launch_pass(plan->host.passes[pass_index], &plan->cache[pass_index], device_state,
+    cudaError_t e = qft_launch_pass(plan->host.passes[pass_index], &plan->cache[pass_index], device_state, device_state,
                                     (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return QFT_OK;

@@ -277,7 +277,10 @@ static bool encode_map(const QftPassDesc& d, void* state, CUtensorMap* map) {
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int dev, void* state, cudaStream_t stream) {
+// src: the buffer the tile loads come from (the tensor map's base); state: the buffer the stores go to.  They differ
+// only for the first pass of an out-of-place execute.
+static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int dev, void* src, void* state,
+                               cudaStream_t stream) {
     tma2_kernel_t kern = pick_tma2(d);
     if (!kern) return cudaErrorNotSupported;
     const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb, d.ntile);
@@ -286,12 +289,12 @@ static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int de
         std::lock_guard<std::mutex> lock(cache->mu);
         const QftPassCache::Entry* hit = nullptr;
         for (const auto& e : cache->maps)
-            if (e.ptr == state && e.dev == dev) hit = &e;
+            if (e.ptr == src && e.dev == dev) hit = &e;
         if (hit) {
             map = hit->map;
         } else {
-            if (!encode_map(d, state, &map)) {
-                if (d.xt) return cudaErrorNotSupported;
+            if (!encode_map(d, src, &map)) {
+                if (d.xt || src != state) return cudaErrorNotSupported;
                 // no tensor map: the generic kernel runs the same descriptor (F = Fst for every plain pass)
                 QftPassDesc g = d;
                 g.kernel = QFT_KERNEL_GENERIC;
@@ -302,7 +305,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int de
             }
             QftPassCache::Entry& e = cache->maps[cache->next];
             cache->next = (cache->next + 1) % 4;
-            e.ptr = state;
+            e.ptr = src;
             e.dev = dev;
             e.map = map;
         }
@@ -343,11 +346,14 @@ static cudaError_t launch_tma2(const QftPassDesc& d, QftPassCache* cache, int de
     return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
 }
 
-cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* state, cudaStream_t stream) {
+bool qft_pass_reads_through_tensor_map(const QftPassDesc& d) { return d.kernel == QFT_KERNEL_TMA2; }
+
+cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* src, void* state, cudaStream_t stream) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    if (d.kernel == QFT_KERNEL_TMA2) return launch_tma2(d, cache, dev, state, stream);
+    if (d.kernel == QFT_KERNEL_TMA2) return launch_tma2(d, cache, dev, src, state, stream);
+    if (src != state) return cudaErrorNotSupported;
     std::lock_guard<std::mutex> lock(cache->mu);
     return launch_plain(d, cache, dev, state, stream);
 }

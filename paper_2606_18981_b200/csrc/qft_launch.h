@@ -21,4 +21,7 @@ struct QftPassCache {
     } maps[4];
 };
 
-cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* state, cudaStream_t stream);
+// Enqueue one pass: tiles are loaded from `src` and stored to `state` (the same buffer for an in-place pass; a
+// different one only if qft_pass_reads_through_tensor_map(d), else cudaErrorNotSupported).
+cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* src, void* state, cudaStream_t stream);
+bool qft_pass_reads_through_tensor_map(const QftPassDesc& d);

@@ -164,32 +164,56 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) 
 bool build_deferred(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) {
     if (n <= fmax) return false;
     const int w = std::min(wcap, fmax - l);
-    if (w < l || w < 1) return false;
-    const int K = ilog2_ceil_div(n, w);
-    if (K < 2) return false;
-    std::vector<int> sizes = split_balanced(n, K);
-    if (sizes.back() < l || sizes.front() < l) return false;
+    if (w < 1 || n < 2 * l) return false;
     const int f = fmax;
-    int t = n - 1;
-    for (int p = 0; p < K; ++p) {
+    // address of qubit q once the hub has traded places with the top l bits
+    auto addr_after = [&](int q) { return (q < l || q >= n - l) ? n - 1 - q : q; };
+    auto window_pass = [&](int t, int size, bool swapped, bool natural_run) {
         PassSpec ps;
-        for (int i = 0; i < sizes[p]; ++i) ps.window.push_back(t - i);
-        const int lo = t - sizes[p] + 1;
         std::set<int> F;
         for (int a = 0; a < l; ++a) F.insert(a);
-        if (p == K - 1) {
-            // qubits lo .. l sit on their own addresses, qubits l-1 .. 0 on the top l addresses (reversed)
-            for (int a = l; a <= t; ++a) F.insert(a);
-            for (int a = n - l; a < n; ++a) F.insert(a);
-        } else {
-            for (int a = lo; a <= t; ++a) F.insert(a);
+        for (int i = 0; i < size; ++i) {
+            ps.window.push_back(t - i);
+            F.insert(swapped ? addr_after(t - i) : t - i);
         }
         ps.F.assign(F.begin(), F.end());
-        if (p == 0)
-            for (int a = 0; a < l; ++a) { ps.moves.push_back({a, n - 1 - a}); ps.moves.push_back({n - 1 - a, a}); }
-        if (p > 0 && p < K - 1) ps.extras_above = t;
+        if (natural_run) ps.extras_above = t;
+        return ps;
+    };
+    std::vector<int> sizes = split_balanced(n, ilog2_ceil_div(n, w));
+    if (sizes.size() >= 2 && sizes.front() >= l && sizes.back() >= l) {
+        // the first pass holds the top l qubits next to the hub: it trades them
+        int t = n - 1;
+        for (size_t p = 0; p < sizes.size(); ++p) {
+            PassSpec ps = window_pass(t, sizes[p], p > 0, p > 0 && p + 1 < sizes.size());
+            if (p == 0)
+                for (int a = 0; a < l; ++a) { ps.moves.push_back({a, n - 1 - a}); ps.moves.push_back({n - 1 - a, a}); }
+            add_extras(ps, n, f);
+            t -= sizes[p];
+            out->push_back(ps);
+        }
+        return true;
+    }
+    // windows smaller than the hub: process the top l qubits where they sit, trade hub and top in a pass of its own
+    // (permutation only), then process the rest
+    int t = n - 1;
+    for (int sz : split_balanced(l, ilog2_ceil_div(l, w))) {
+        PassSpec ps = window_pass(t, sz, false, false);
         add_extras(ps, n, f);
-        t -= sizes[p];
+        t -= sz;
+        out->push_back(ps);
+    }
+    {
+        PassSpec ps;
+        for (int a = 0; a < l; ++a) { ps.F.push_back(a); ps.moves.push_back({a, n - 1 - a}); ps.moves.push_back({n - 1 - a, a}); }
+        for (int a = n - l; a < n; ++a) ps.F.push_back(a);
+        add_extras(ps, n, f);
+        out->push_back(ps);
+    }
+    for (int sz : split_balanced(n - l, ilog2_ceil_div(n - l, w))) {
+        PassSpec ps = window_pass(t, sz, true, false);
+        add_extras(ps, n, f);
+        t -= sz;
         out->push_back(ps);
     }
     return true;
@@ -727,7 +751,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
                 specs.back().moves.clear();
             } else if (!build_deferred(n, prm.max_fused, fplan, l, &specs)) {
                 if (attempt == 0) continue;
-                *err = "deferred swaps: windows smaller than the hub cannot be scheduled";
+                *err = "deferred swaps: this tile / hub combination cannot be scheduled";
                 return 2;
             }
             out->folded = true;  // no stand-alone permutation pass

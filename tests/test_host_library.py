@@ -128,3 +128,96 @@ def test_k_is_clamped_and_reported():
     assert p.describe()["k"] == 12
     assert p.gate_counts()[1] == 66
     p.close()
+
+
+def test_deferred_swaps_plans():
+    """QFT_FLAG_DEFER_SWAPS: the host proof holds for every n, the reported layout is a permutation of the qubits, no
+    pass exchanges tiles between CTAs, and there are never more passes than with the swaps applied."""
+    for n in range(1, 35):
+        for w in (13, 4):
+            p = qft.Plan(n, 6, w, flags=qft.QFT_FLAG_DEFER_SWAPS)
+            p.self_check()
+            d = p.describe()
+            assert d["swaps"] == "deferred"
+            assert sorted(p.output_order()) == list(range(n))
+            assert all(not ps["pair_swaps"] for ps in d["passes"])
+            q = qft.Plan(n, 6, w)
+            assert q.output_order() == [n - 1 - a for a in range(n)] and q.describe()["swaps"] == "applied"
+            if w == 13:
+                assert p.num_passes <= q.num_passes
+            p.close()
+            q.close()
+    with pytest.raises(qft.QftError) as ei:
+        qft.qft_plan_create_batched(12, 4, 12, 13, -1, 0)  # sanity: batched plans exist ...
+        qft.qft_plan_create_tuned(12, 12, 13, -1, 0, 0, 0, qft.QFT_FLAG_DEFER_SWAPS | qft.QFT_FLAG_UNFOLDED)
+    assert ei.value.status == qft.QFT_ERR_UNSUPPORTED
+
+
+def test_passes_name_their_gates():
+    """PAPER.md:145 / :147: every fused block records the contiguous sub-range of the time-ordered gate list it folds.
+    The ranges must tile the list [0, n_h + n_cr) in order, and their H / CR counts must add up to the plan's counters,
+    i.e. to Table 2's seven rows at n = 22."""
+    table2 = {21: 231, 16: 216, 12: 186, 10: 165, 8: 140, 6: 111, 4: 78}
+    for k, n_cr in table2.items():
+        for w, flags in ((13, 0), (3, 0), (13, qft.QFT_FLAG_UNFOLDED), (5, qft.QFT_FLAG_DEFER_SWAPS)):
+            p = qft.Plan(22, k, w, flags=flags)
+            d = p.describe()
+            nxt, th, tc = 0, 0, 0
+            for ps in d["passes"]:
+                if ps["n_h"] == 0:
+                    assert ps["gate_first"] == -1 and not ps["window"]  # permutation only: part of the swap network
+                    continue
+                assert ps["gate_first"] == nxt and ps["gate_last"] == nxt + ps["n_h"] + ps["n_cr"] - 1
+                assert ps["n_h"] == len(ps["window"])
+                assert ps["n_cr"] == sum(min(k, t) for t in ps["window"])
+                nxt = ps["gate_last"] + 1
+                th += ps["n_h"]
+                tc += ps["n_cr"]
+            assert (th, tc) == (22, n_cr) and nxt == 22 + n_cr
+            assert p.gate_counts() == (22, n_cr, 11)
+            p.close()
+    # the n = 30 bench plan: three fused blocks of 10 Hadamards each
+    p = qft.Plan(30, 30)
+    assert [(ps["n_h"], ps["n_cr"]) for ps in p.describe()["passes"]] == [(10, 245), (10, 145), (10, 45)]
+    p.close()
+
+
+def test_unschedulable_tuning_is_unsupported_not_internal():
+    """tile_bits < 2 * hub_bits cannot hold the hub beside a window (or twice, in the stand-alone
+    reversal tile); qft.h promises QFT_ERR_UNSUPPORTED for that, never QFT_ERR_INTERNAL."""
+    for tile_bits, hub_bits in ((3, 2), (4, 3), (5, 3), (5, 4), (6, 4), (7, 4), (8, 5), (9, 5)):
+        for flags in (0, qft.QFT_FLAG_UNFOLDED):
+            with pytest.raises(qft.QftError) as ei:
+                qft.qft_plan_create_tuned(20, 20, 13, -1, 0, tile_bits, hub_bits, flags)
+            assert ei.value.status == qft.QFT_ERR_UNSUPPORTED
+    # fuzz: whatever the knobs, the planner answers ok / unsupported / invalid, never "internal"
+    import random
+
+    rng = random.Random(5)
+    for _ in range(1500):
+        n, t, h = rng.randint(1, 34), rng.randint(0, 15), rng.randint(0, 7)
+        w, fl = rng.randint(1, 14), rng.choice([0, 1, 2, 4, 16, 32, 6, 17, 33])
+        try:
+            qft.qft_plan_destroy(qft.qft_plan_create_tuned(n, rng.randint(0, 40), w, -1, 0, t, h, fl))
+        except qft.QftError as e:
+            assert e.status in (qft.QFT_ERR_UNSUPPORTED, qft.QFT_ERR_INVALID_ARG), (n, t, h, w, fl, str(e))
+
+
+def test_describe_length_and_small_buffers():
+    import ctypes
+
+    L = qft.load()
+    p = qft.Plan(34, 34, 1)  # 35 passes: the longest description
+    need = qft.qft_plan_describe_length(p.handle)
+    assert need > 8192
+    small = ctypes.create_string_buffer(need - 1)
+    assert L.qft_plan_describe(p.handle, small, need - 1) == qft.QFT_ERR_INVALID_ARG
+    exact = ctypes.create_string_buffer(need)
+    assert L.qft_plan_describe(p.handle, exact, need) == qft.QFT_OK and len(exact.value) == need - 1
+    assert qft.qft_plan_describe_length(None) == 0
+    p.close()
+
+
+def test_num_qubits_for_length():
+    assert [qft.qft_num_qubits_for(v) for v in (1, 2, 3, 4, 5, 1000, 1024, 1025)] == [1, 1, 2, 2, 3, 10, 10, 11]
+    assert qft.qft_num_qubits_for(0) == -1 and qft.qft_num_qubits_for((1 << 34) + 1) == -1

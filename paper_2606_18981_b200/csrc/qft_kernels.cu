@@ -180,10 +180,21 @@ tma2_kernel_t qft_pick_tma2_lt7(int r1, int r2, int kc);  // qft_tma_lt7.cu
 tma2_kernel_t qft_pick_tma2_lt8(int r1, int r2, int kc);  // qft_tma_lt8.cu
 tma2_kernel_t qft_pick_tma2_lt9(int r1, int r2, int kc);  // qft_tma_lt9.cu
 tma2_kernel_t qft_pick_tma2_xt(int r1, int r2, int kc);   // qft_tma_xt.cu
+tma2_kernel_t qft_pick_tma2_es7(int r1, int r2, int kc);  // qft_tma_es.cu
+tma2_kernel_t qft_pick_tma2_es8(int r1, int r2, int kc);
+tma2_kernel_t qft_pick_tma2_es9(int r1, int r2, int kc);
 
 static tma2_kernel_t pick_tma2(const QftPassDesc& d) {
     const int kc = d.k < 4 ? d.k : 4;
     if (d.xt) return d.log2_threads == 9 ? qft_pick_tma2_xt(d.tma.r1, d.tma.r2, kc) : nullptr;
+    if (d.tma.eb > QFT_TMA2_EB_DIRECT) {
+        switch (d.log2_threads) {
+            case 7: return qft_pick_tma2_es7(d.tma.r1, d.tma.r2, kc);
+            case 8: return qft_pick_tma2_es8(d.tma.r1, d.tma.r2, kc);
+            case 9: return qft_pick_tma2_es9(d.tma.r1, d.tma.r2, kc);
+        }
+        return nullptr;
+    }
     switch (d.log2_threads) {
         case 7: return qft_pick_tma2_lt7(d.tma.r1, d.tma.r2, kc);
         case 8: return qft_pick_tma2_lt8(d.tma.r1, d.tma.r2, kc);

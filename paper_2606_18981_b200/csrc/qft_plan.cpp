@@ -98,15 +98,23 @@ void build_unfolded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out
 
 // Folded schedule: K = 2 + #mid passes, no stand-alone reversal.
 //   regions: H=[0,l)  A=[l,we)  Mid=[we,n-we)  B=[n-we,n-l)  T=[n-l,n)
-bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) {
+//   we_force > 0: that width for the first and the last window instead of the balanced one.
+bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out, int we_force = 0) {
     if (n <= fmax) return false;
     int w = std::min(wcap, fmax - l);
     if (n <= 2 * w) w = (n - 1) / 2;
     if (w < l || w < 1) return false;
-    int nmid_passes = ilog2_ceil_div(n - 2 * w, w);
-    const int K = 2 + nmid_passes;
-    int we = std::min(w, ilog2_ceil_div(n, K));
-    while (n - 2 * we > nmid_passes * w) ++we;
+    int nmid_passes, we;
+    if (we_force > 0) {
+        we = we_force;
+        if (we > w || n - 2 * we < 1) return false;
+        nmid_passes = ilog2_ceil_div(n - 2 * we, w);
+    } else {
+        nmid_passes = ilog2_ceil_div(n - 2 * w, w);
+        const int K = 2 + nmid_passes;
+        we = std::min(w, ilog2_ceil_div(n, K));
+        while (n - 2 * we > nmid_passes * w) ++we;
+    }
     if (we < l || n - 2 * we < 1) return false;
     const int nmid = n - 2 * we;
     std::vector<int> chunks = split_balanced(nmid, nmid_passes);
@@ -150,6 +158,52 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out) 
         for (int a = n - we; a < n; ++a) ps.F.push_back(a);
         add_extras(ps, n, f);
         out->push_back(ps);
+    }
+    return true;
+}
+
+// max_fused_qubits smaller than the hub (PAPER.md:145's cap on the fused size; BASELINE config 3 sweeps it down to 2):
+// no window can hold the hub's partner bits, so the folded schedule is laid out for the widest window the tile allows
+// and every one of its windows is cut into sub-passes of <= wcap qubits.  Only the last sub-pass of a window carries
+// the window's layout adapter (in-tile moves, pair involution); the others run in place on a tile of their own:
+// hub + sub-window + the lowest free address bits, i.e. long contiguous rows.
+bool build_folded_split(int n, int wcap, int fmax, int l, int we, std::vector<PassSpec>* out) {
+    std::vector<PassSpec> sup;
+    if (!build_folded(n, fmax - l, fmax, l, &sup, we)) return false;
+    std::vector<int> qubit_at(n);
+    for (int a = 0; a < n; ++a) qubit_at[a] = a;
+    for (const PassSpec& sp : sup) {
+        const int W = (int)sp.window.size();
+        // smaller sub-windows first: a one-qubit window (only the generic kernel takes it) then runs in place on a small tile
+        std::vector<int> sizes = split_balanced(W, ilog2_ceil_div(W, wcap));
+        std::reverse(sizes.begin(), sizes.end());
+        int off = 0;
+        for (size_t c = 0; c < sizes.size(); ++c) {
+            std::vector<int> win(sp.window.begin() + off, sp.window.begin() + off + sizes[c]);
+            off += sizes[c];
+            PassSpec s;
+            if (c + 1 == sizes.size()) {
+                s = sp;
+            } else {
+                std::set<int> F;
+                for (int a = 0; a < l; ++a) F.insert(a);
+                for (int q : win) {
+                    int at = -1;
+                    for (int a = 0; a < n; ++a)
+                        if (qubit_at[a] == q) at = a;
+                    if (at < l) return false;  // a window qubit never sits on a hub bit when its turn comes
+                    F.insert(at);
+                }
+                s.F.assign(F.begin(), F.end());
+                add_extras(s, n, fmax);
+            }
+            s.window = win;
+            out->push_back(s);
+        }
+        std::vector<int> nq(qubit_at);
+        for (auto& m : sp.moves) nq[m.second] = qubit_at[m.first];
+        for (auto& sw : sp.swaps) { nq[sw.first] = qubit_at[sw.second]; nq[sw.second] = qubit_at[sw.first]; }
+        qubit_at.swap(nq);
     }
     return true;
 }
@@ -307,7 +361,8 @@ void lower_tma2(QftPassDesc* d, int n) {
     if (d->xt && (f != 14 || r1 + r2 < 8)) QFT_REJECT(4);  // the extended tile is built for 2^14 halves only
     if (s1.a != s2.a + r2) QFT_REJECT(5);  // the window is one run of canonical bits
     const int eb = s2.a;            // canonical bits below the window
-    if (eb > 7) QFT_REJECT(6);
+    // more than QFT_TMA2_EB_DIRECT: the split end table, instantiated for windows of <= 6 qubits (qft_tma_es*.cu)
+    if (eb > QFT_TMA2_EB_MAX || (eb > QFT_TMA2_EB_DIRECT && (r1 + r2 > 6 || d->xt))) QFT_REJECT(6);
     if (n - f < 1) QFT_REJECT(7);
     QftTma2Desc t;
     std::memset(&t, 0, sizeof t);
@@ -420,14 +475,14 @@ void lower_tma2(QftPassDesc* d, int n) {
         return slot << 3;
     };
     auto landcol = [&](int c) -> uint32_t { return 8u << land_idx_of_canon[c]; };
-    auto key1 = [&](int c) -> uint16_t {
-        if (in2(c)) return (uint16_t)(1u << (c - s2.a));
-        if (c < eb) return (uint16_t)(1u << (8 + c));
+    auto key1 = [&](int c) -> uint32_t {
+        if (in2(c)) return 1u << (c - s2.a);
+        if (c < eb) return 1u << (8 + c);
         return 0;
     };
-    auto key2 = [&](int c) -> uint16_t {
-        if (in1(c)) return (uint16_t)(1u << (c - s1.a));
-        if (c < eb) return (uint16_t)(1u << (8 + c));
+    auto key2 = [&](int c) -> uint32_t {
+        if (in1(c)) return 1u << (c - s1.a);
+        if (c < eb) return 1u << (8 + c);
         return 0;
     };
     for (int j = 0; j < lt; ++j) {
@@ -684,6 +739,12 @@ static bool lower_all(const QftPlanParams& prm, std::vector<PassSpec>& specs, in
                 done = true;
             }
         }
+        // a one-qubit window that only the generic kernel takes, in place: a small tile (many CTAs per SM) instead of
+        // the plan's large one
+        if (!done && ps.window.size() == 1 && ps.moves.empty() && ps.swaps.empty() && !ps.Fbase.empty() && na > fsmem) {
+            const int ft = std::max(fbase, std::min((int)ps.F.size(), 11));
+            if (ft < (int)ps.F.size()) add_extras(ps, na, ft);
+        }
         if (!done && !lower_pass(ps, na, k_eff, conj, l, allow_fused, allow_tma, qubit_at, &d, err)) return false;
         wmaxseen = std::max(wmaxseen, (int)ps.window.size());
         out->passes.push_back(d);
@@ -735,7 +796,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     out->n_swap = n / 2;
 
     // tensor-memory extended tiles (one more window qubit per pass than the shared-memory tile holds): only for
-    // 2^14 tiles (two CTAs per SM on 2^13 halves measured slower: profiles/r02_ext_tile.md), single transforms, TMA
+    // 2^14 tiles (one 512-thread CTA per SM; the kernel is instantiated for that shape only), single transforms, TMA
     // kernels allowed; tried first, dropped if any pass cannot be lowered
     const bool ext_ok = fmax == 14 && prm.batch_bits == 0 && !(prm.flags & (1u | 2u | 4u | 16u)) && n > fmax + 1;
     if ((prm.flags & 32u) && prm.batch_bits != 0) { *err = "deferred swaps are not available for batched plans"; return 2; }
@@ -776,6 +837,47 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
             break;
         }
         if (attempt == 1) { *err = e2; return 5; }
+    }
+    if (!(prm.flags & (1u | 2u | 4u | 16u | 32u)) && prm.max_fused <= 6 && prm.max_fused < fmax - l && n > fmax) {
+        // Small windows (PAPER.md:145's cap on the fused size; BASELINE config 3 sweeps it down to 2): besides the
+        // schedule above (if it exists), cut the folded schedule's windows into sub-passes.  For every hub size
+        // (unless the caller fixed it) and width of the outer windows, lower the candidate and keep the cheapest
+        // by a rough per-pass cost of the kernel each pass ended up with.
+        auto pass_cost = [](const QftPassDesc& d) -> long {
+            return d.kernel == QFT_KERNEL_TMA2 ? (d.npair || d.f < 13 ? 12 : 10) : d.kernel == QFT_KERNEL_FUSED2 ? 25 : (d.f >= 10 && d.f <= 11 && !d.npair ? 40 : 100);
+        };
+        auto cost_of = [&](std::vector<PassSpec>& cand, int lh, QftHostPlan* tmp) -> long {
+            *tmp = *out;
+            tmp->passes.clear();
+            tmp->hub_bits = lh;
+            if (na > n)
+                for (auto& ps : cand) add_extras(ps, na, std::min(fmax, na));
+            std::string e3;
+            if (!lower_all(prm, cand, na, out->k_eff, lh, fmax, tmp, &e3)) return -1;
+            long c = 0;
+            for (const QftPassDesc& d : tmp->passes) c += pass_cost(d);
+            return c;
+        };
+        QftHostPlan best_plan, tmp;
+        long best = 0;  // the cost of the schedule found above
+        for (const QftPassDesc& d : out->passes) best += pass_cost(d);
+        const long native = best;
+        for (int lh = l; lh >= (prm.hub_bits ? l : 3) && lh >= 1; --lh)
+            for (int we = lh; we <= fmax - lh; ++we) {
+                std::vector<PassSpec> cand;
+                if (!build_folded_split(n, prm.max_fused, fmax, lh, we, &cand)) continue;
+                if ((long)cand.size() * 10 >= best) continue;  // cannot win
+                const long c = cost_of(cand, lh, &tmp);
+#ifdef QFT_PLAN_DEBUG
+                fprintf(stderr, "split candidate hub %d we %d: %zu passes, cost %ld\n", lh, we, cand.size(), c);
+#endif
+                if (c >= 0 && c < best) { best = c; best_plan = tmp; }
+            }
+        if (best < native) {
+            *out = best_plan;
+            out->folded = true;
+            out->ext_tile = false;
+        }
     }
     // normalisation: every H contributes 1/sqrt 2; applied once, in the last pass
     double sc = std::pow(2.0, -0.5 * n);
@@ -928,7 +1030,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     uint32_t kb = key;
                     for (int b = s1.r; b < 5; ++b) if ((B >> b) & 1) kb ^= t.s1_reg_key[b];
                     if ((kb & 31u) != ((c >> s2.a) & ((1u << s2.r) - 1u))) return fail("tma2: step 1 key (group 2 value)");
-                    if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
+                    if (((kb >> 8) & 4095u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 1 key (e)");
                     if (offm & 7u) return fail("tma2: mid offset alignment");
                     const uint32_t slot = offm >> 3;
                     if (slot >= xslots || mid_canon[slot] != -1) return fail("tma2: exchange layout is not a bijection");
@@ -986,7 +1088,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                     const uint32_t c = (uint32_t)mid_canon[slot];
                     if (((c >> s2.a) & ((1u << s2.r) - 1u)) != (uint32_t)(B & ((1 << s2.r) - 1))) return fail("tma2: step 2 register bits");
                     if ((kb & 31u) != ((c >> s1.a) & ((1u << s1.r) - 1u))) return fail("tma2: step 2 key (group 1 value)");
-                    if (((kb >> 8) & 127u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
+                    if (((kb >> 8) & 4095u) != (c & ((1u << t.eb) - 1u))) return fail("tma2: step 2 key (e)");
                     // the element with canonical index c must land on store-order index st(c)
                     uint32_t want = 0;
                     for (int j = 0; j < f; ++j) if ((c >> d.st_canon[j]) & 1u) want |= 1u << j;
@@ -996,7 +1098,7 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
                 }
             }
             for (int j = 0; j < std::min<int>(t.tma_box[0], 3) && j < lt; ++j) if (t.s2_tid_addr[j] != d.Fst[j] || d.Fst[j] != j) return fail("tma2: store lanes do not run along the hub");
-            if (t.eb != s2.a || t.eb > 7) return fail("tma2: eb");
+            if (t.eb != s2.a || t.eb > QFT_TMA2_EB_MAX || (t.eb > QFT_TMA2_EB_DIRECT && (s1.r + s2.r > 6 || d.xt))) return fail("tma2: eb");
             for (int c = 0; c < t.eb; ++c) if (t.e_log[c] != d.log_canon[c]) return fail("tma2: e_log");
             if (t.t1_lo != s1.t_hi - s1.r + 1 || t.t2_lo != s2.t_hi - s2.r + 1 || t.t1_lo != t.t2_lo + s2.r) return fail("tma2: group qubits");
             if (t.r1 != s1.r || t.r2 != s2.r) return fail("tma2: group sizes");

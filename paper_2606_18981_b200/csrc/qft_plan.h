@@ -22,12 +22,20 @@
 #define QFT_MAX_TILEIDX_BITS 34
 #define QFT_MAX_STEPS 14
 #define QFT_MAX_RADIX_BITS 5
-// QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, 2 x 32 rows of end bases, one mbarrier,
-// 5 coords + the tensor-memory base address
+// QFT_KERNEL_TMA2 shared-memory tables after the tile: 32 rows of mid bases, two per-tile end tables (by parity)
+// of 2^eb rows (at least 32), one mbarrier, 5 coords + the tensor-memory base address, the tile-index byte tables.
+// More than QFT_TMA2_EB_DIRECT in-tile qubits below the window ("split end table", small windows high up in a large
+// tile): the per-tile tables cover the lowest QFT_TMA2_EB_LO of them and one table that is constant for the whole
+// launch covers the rest; the kernel multiplies the two factors.
 #define QFT_TMA2_MID_STRIDE 9   // float2 per row (<= 5 used; odd: rows of different lanes fall into different banks)
 #define QFT_TMA2_END_STRIDE 17  // float2 per row (R1 + R2 + 1 <= 11 used; odd for the same reason)
+#define QFT_TMA2_EB_DIRECT 7
+#define QFT_TMA2_EB_LO 6
+#define QFT_TMA2_EB_MAX 12
+#define QFT_TMA2_END_ROWS(eb) \
+    ((eb) > QFT_TMA2_EB_DIRECT ? 2 * (1 << QFT_TMA2_EB_LO) + (1 << ((eb)-QFT_TMA2_EB_LO)) : 2 * ((eb) > 5 ? (1 << (eb)) : 32))
 #define QFT_TMA2_TABLE_BYTES(eb, ntile) \
-    ((32 * QFT_TMA2_MID_STRIDE + 2 * ((eb) > 5 ? (1 << (eb)) : 32) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24 + (((ntile) + 7) >> 3) * 256 * 16)
+    ((32 * QFT_TMA2_MID_STRIDE + QFT_TMA2_END_ROWS(eb) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24 + (((ntile) + 7) >> 3) * 256 * 16)
 
 struct QftStep {
     int8_t r;     // qubits in the group
@@ -50,11 +58,11 @@ struct QftTma2Desc {
     uint32_t s1_tid_ld[9], s1_reg_ld[5];    // step 1 read: the TMA landing layout (tile load order)
     uint32_t s1_tid_mid[9], s1_reg_mid[5];  // step 1 write: the swizzled exchange layout
     uint32_t s2_tid_mid[9], s2_reg_mid[5];  // step 2 read: the same layout seen from step 2's threads
-    uint16_t s1_tid_key[9], s1_reg_key[5];  // step 1 key: bits 0-4 = value of group 2's qubits, 8-14 = e
-    uint16_t s2_tid_key[9], s2_reg_key[5];  // step 2 key: bits 0-4 = value of group 1's qubits, 8-14 = e
+    uint32_t s1_tid_key[9], s1_reg_key[5];  // step 1 key: bits 0-4 = value of group 2's qubits, 8-19 = e
+    uint32_t s2_tid_key[9], s2_reg_key[5];  // step 2 key: bits 0-4 = value of group 1's qubits, 8-19 = e
     int8_t s2_tid_addr[9], s2_reg_addr[5];  // step 2 store: HBM address bit of each thread / register bit
-    int8_t eb;                              // in-tile logical qubits below the window (<= 7); e indexes them
-    int8_t e_log[7];                        // their logical ids, ascending
+    int8_t eb;                              // in-tile logical qubits below the window (<= 12); e indexes them
+    int8_t e_log[QFT_TMA2_EB_MAX];          // their logical ids, ascending
     int8_t t1_lo, t2_lo;                    // lowest logical qubit of group 1 / group 2
     int8_t r1, r2;
     int8_t tma_lo[5], tma_len[5], tma_box[5];  // tensor-map dims: address bits [lo, lo+len), box 2^box

@@ -176,7 +176,7 @@ struct BatchApply {
 #define QFT_PHASE(i)
 #endif
 
-template <int R1, int R2, int KC, int LT, int XT>
+template <int R1, int R2, int KC, int LT, int XT, int ES = 0>
 __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     qft_pass_tma2(float2* __restrict__ state, const __grid_constant__ CUtensorMap tmap,
                   const __grid_constant__ QftPassDesc d) {
@@ -190,10 +190,16 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     float2* endW = reinterpret_cast<float2*>(nextc + 6);     // two end tables (by parity) of max(32, 2^eb) rows
     const uint32_t tid = threadIdx.x;
     const QftTma2Desc& t = d.tma;
-    const uint32_t end_rows = t.eb > 5 ? (1u << t.eb) : 32u;
+    // split end table (ES = 1, more than QFT_TMA2_EB_DIRECT in-tile qubits below the window): the per-tile tables
+    // cover the lowest QFT_TMA2_EB_LO of them, the constant table endHi the rest (the phase is linear over
+    // disjoint bit sets, so a factor is the product of the two entries)
+    const int eb_lo = ES ? QFT_TMA2_EB_LO : t.eb;
+    const uint32_t end_rows = eb_lo > 5 ? (1u << eb_lo) : 32u;
+    float2* endHi = endW + 2 * end_rows * kEndStride;
+    const uint32_t hi_rows = ES ? (1u << (t.eb - QFT_TMA2_EB_LO)) : 0u;
     // tile-index byte -> address bits (tblA) and logical qubit bits (tblL): 256 entries per byte of the tile index
     const int nslice = (d.ntile + 7) >> 3;
-    uint64_t* tblA = reinterpret_cast<uint64_t*>(endW + 2 * end_rows * kEndStride);
+    uint64_t* tblA = reinterpret_cast<uint64_t*>(endHi + hi_rows * kEndStride);
     uint64_t* tblL = tblA + nslice * 256;
 
     // ---- per-thread constants ----
@@ -217,7 +223,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     const int win_lo = d.win_lo;
     // this thread's entry of the per-tile end table (see the tile walk): row e, column q, target qubit, the bits
     // below it that may hold controls, and the phase its own row bits e contribute
-    const uint32_t end_cnt = (uint32_t)NQ << t.eb;
+    const uint32_t end_cnt = (uint32_t)NQ << eb_lo;
     const uint32_t end_e = tid / NQ, end_q = tid % NQ;
     const uint32_t end_slot = end_e * kEndStride + end_q;
     const int end_tq = (XT && end_q == (uint32_t)(R1 + R2)) ? win_lo - 1 : win_lo + (int)end_q;
@@ -225,7 +231,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     uint32_t end_ph_e;
     {
         uint64_t Le = 0;
-        for (int b = 0; b < t.eb; ++b)
+        for (int b = 0; b < eb_lo; ++b)
             if ((end_e >> b) & 1u) Le |= 1ull << t.e_log[b];
         end_ph_e = qftp::cr_phase_u32(Le & end_mask, end_tq > 0 ? end_tq : 0, k);
     }
@@ -252,6 +258,16 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
         for (int q = 0; q < R1; ++q)
             if ((u1 >> q) & 1u) ph += qftp::cr_phase_u32(1ull << (t.t2_lo + (int)b), t.t1_lo + q, k);
         midW[u1 * kMidStride + b] = qftp::cis_fwd_u32(ph);
+    }
+    if constexpr (ES) {
+        // the constant half of the split end table: rows = values of the in-tile qubits e_log[EB_LO ...]
+        for (uint32_t i = tid; i < (uint32_t)NQ * hi_rows; i += NT) {
+            const uint32_t e = i / NQ, q = i % NQ;
+            uint64_t L = 0;
+            for (int b = QFT_TMA2_EB_LO; b < t.eb; ++b)
+                if ((e >> (b - QFT_TMA2_EB_LO)) & 1u) L |= 1ull << t.e_log[b];
+            endHi[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, win_lo + (int)q, k));
+        }
     }
     for (int i = (int)tid; i < nslice * 256; i += NT) {
         uint64_t a = 0, L = 0;
@@ -338,7 +354,7 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
                 for (uint32_t i = tid + NT; i < end_cnt; i += NT) {  // only when 2^eb (R1 + R2 + XT) > threads
                     const uint32_t e = i / NQ, q = i % NQ;
                     uint64_t L = Ltile;
-                    for (int b = 0; b < t.eb; ++b)
+                    for (int b = 0; b < eb_lo; ++b)
                         if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
                     int tq = win_lo + (int)q;
                     if (XT && q == (uint32_t)(R1 + R2)) tq = win_lo - 1;
@@ -424,13 +440,14 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
 #pragma unroll
                 for (int i = 0; i < 5 - R2; ++i)
                     if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
-                const float2* row = endWp + ((kk >> 8) & 127u) * kEndStride;
+                const float2* row = endWp + ((kk >> 8) & (ES ? 63u : 127u)) * kEndStride;
+                const float2* rowh = endHi + ((kk >> (8 + QFT_TMA2_EB_LO)) & 63u) * kEndStride;  // ES only
 #pragma unroll
-                for (int i = 0; i < R2; ++i) W2[bt][i] = row[i];
+                for (int i = 0; i < R2; ++i) W2[bt][i] = ES ? qftp::cmul(row[i], rowh[i]) : row[i];
                 float2 c = make_float2(d.scale, 0.f);
 #pragma unroll
                 for (int i = 0; i < R1; ++i) {
-                    const float2 w = row[R2 + i];
+                    const float2 w = ES ? qftp::cmul(row[R2 + i], rowh[R2 + i]) : row[R2 + i];
                     const float2 cw = qftp::cmul(c, w);
                     if ((kk >> i) & 1u) c = cw;
                 }

@@ -166,3 +166,36 @@ def test_execute_is_cuda_graph_capturable():
     got = t.cpu().numpy().astype(np.complex128)
     assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 2e-5
     plan.close()
+
+
+# Small max_fused_qubits (BASELINE config 3 sweeps it down to 2): the planner cuts the folded schedule's windows into
+# sub-passes that run on large tiles, so a small window high up in the tile sees up to 12 in-tile qubits below it
+# (the split end table of the TMA kernel: more than 7).  Every sub-window shape (1+1, 2+1, 2+2, 3+2, 3+3), three tile
+# sizes, exact and truncated rotations, both signs.
+@pytest.mark.parametrize("n,tile_bits", [(18, 12), (20, 13), (21, 13), (22, 14), (23, 12), (24, 14)])
+@pytest.mark.parametrize("w", [2, 3, 4, 5, 6])
+def test_small_windows_against_oracle(n, tile_bits, w):
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    x = qi.gaussian(n, 100 + n)
+    deepest = 0
+    for k, sign, norm in [(None, -1, 0), (3, 1, 1), (1, -1, 0), (7, -1, 2)]:
+        kk = n if k is None else k
+        plan = qft.Plan(n, kk, w, sign, norm, tile_bits, 0, 0)
+        plan.self_check()
+        passes = plan.describe()["passes"]
+        kinds = [p["kernel"] for p in passes]
+        assert all(len(p["window"]) <= w for p in passes)
+        for p in passes:
+            if p["kernel"] == "tma2":
+                deepest = max(deepest, sum(1 for q in p["canon_qubits"] if q < min(p["window"])))
+        t = torch.from_numpy(x).cuda()
+        plan.execute(t)
+        torch.cuda.synchronize()
+        got = t.cpu().numpy().astype(np.complex128)
+        plan.close()
+        assert_parity_numpy(got, oracle.qft(x, kk, sign, norm), n, (n, tile_bits, w, kk, sign, norm, kinds))
+    if w <= 4:
+        assert deepest > 7, "this configuration was chosen to exercise the split end table"

@@ -115,12 +115,15 @@ def test_pass_counts_at_the_bench_configs():
         assert p.num_launches == passes
         p.close()
     # config 3: sweep of max_fused_qubits at n = 26
+    # (ceil(26 / w) passes, every one of them in the TMA-staged kernel: small windows are sub-passes of the folded
+    # schedule's windows, not the natural-order schedule with its stand-alone reversal)
     got = []
     for w in (2, 4, 6, 10, 13):
         p = qft.Plan(26, 26, w)
         got.append(p.num_passes)
+        assert {ps["kernel"] for ps in p.describe()["passes"]} == {"tma2"}, w
         p.close()
-    assert got == sorted(got, reverse=True) and got[-1] == 3
+    assert got == [13, 7, 5, 3, 3]
 
 
 def test_k_is_clamped_and_reported():

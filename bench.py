@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--extrapolate-cpu", action="store_true",
                     help="also estimate the oracle's time at the bench n from a few gates (labelled as extrapolated)")
     ap.add_argument("--sweep", default="26,33", help="comma list of extra n to time briefly ('' = none)")
+    ap.add_argument("--small-n", default="20,22", help="comma list of launch-bound sizes to time over 1000 back-to-back "
+                                                       "transforms ('' = none)")
     ap.add_argument("--batched", default="16:12", help="comma list of n:log2_batch pairs to time briefly (batched "
                                                        "plans; '' = none), e.g. 10:18,16:12")
     return ap.parse_args()
@@ -354,6 +356,7 @@ def main():
 
     # ---- per-pass timing for the roofline of the dominant kernel ----
     npass = plan.num_passes
+    nlaunch = plan.num_launches  # kernels one qft_execute enqueues (1 when the plan runs as a single cooperative launch)
     reps = max(3, min(steps, 10))
     acc = [0.0] * npass
     for _ in range(reps):
@@ -503,6 +506,35 @@ def main():
             del r
             torch.cuda.empty_cache()
 
+    # ---- the launch-bound regime (PAPER.md:197's sizes): microseconds per transform over 1000 back-to-back executes ----
+    small = []
+    if args.small_n and rank == 0 and world == 1:
+        torch.cuda.empty_cache()
+        for sn in [int(v) for v in args.small_n.split(",") if v]:
+            row = {"n": sn, "transforms": 1000}
+            for label, fl in (("one_launch", args.flags), ("launch_per_pass", args.flags | qft.QFT_FLAG_MULTI_LAUNCH)):
+                pl = qft.Plan(sn, sn if args.k is None else args.k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
+                              args.hub_bits, fl)
+                stt = torch.empty(1 << sn, dtype=torch.complex64, device="cuda")
+                torch.view_as_real(stt).normal_()
+                stt.mul_(2.0 ** (-(sn + 1) / 2))
+                strm = torch.cuda.current_stream()
+                for _ in range(20):
+                    qft.qft_execute(pl.handle, stt.data_ptr(), strm.cuda_stream)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(strm)
+                for _ in range(1000):
+                    qft.qft_execute(pl.handle, stt.data_ptr(), strm.cuda_stream)
+                e1.record(strm)
+                torch.cuda.synchronize()
+                us = e0.elapsed_time(e1)  # ms for 1000 transforms = microseconds per transform
+                row[label] = {"us_per_transform": us, "launches": pl.num_launches,
+                              "gflops": 5.0 * (1 << sn) * sn / (us * 1e-6) / 1e9}
+                pl.close()
+                del stt
+            small.append(row)
+
     # ---- CPU baseline: the oracle as it stands, WHOLE circuits, rank 0 at N = 1 only ----
     # 1 warm-up + 3 trials, median, at n = 22 (to sit beside PAPER.md:185's 3.86 s / 0.064 s)
     # and n = 26 (the largest size whose whole circuit takes seconds); a bounded sample of the n = 30 workload
@@ -539,7 +571,7 @@ def main():
                              "state fits L2: HBM fraction not meaningful",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "time_ms": ms_per_step, "hbm_gbs": roofline["step_gbs"], "hbm_frac_of_measured_peak": roofline["step_frac"],
-            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline, "gpu_launches": steps * npass,
+            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline, "gpu_launches": steps * nlaunch,
             "clocks": clocks,
         }
         if variants:
@@ -548,6 +580,8 @@ def main():
             line["sweep"] = sweep
         if batched:
             line["batched"] = batched
+        if small:
+            line["small_n"] = small
         print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist

@@ -124,6 +124,12 @@ qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_bat
  * the granule size; callers must read it from the plan, not assume it.  Not available for batched plans.
  */
 #define QFT_FLAG_DEFER_SWAPS 32u
+/* QFT_FLAG_MULTI_LAUNCH -- one kernel launch per pass even where the whole transform would run in one.  By default
+ * a plan whose state lives in L2 (n = 20 ... 24, the paper's measured sizes: Fig. 4) and whose three
+ * passes share a tile size runs as ONE cooperative launch with grid-wide barriers between the passes (no launch gaps,
+ * tables of pass p + 1 built while pass p drains).  qft_plan_num_launches reports which applies; if the device refuses
+ * the cooperative launch (not enough SMs free for the whole grid) the plan silently reverts to one launch per pass. */
+#define QFT_FLAG_MULTI_LAUNCH 64u
 qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                                    qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
 

@@ -5,6 +5,7 @@
 #include <new>
 #include <string>
 
+#include <atomic>
 #include <memory>
 
 #include "../../include/qft.h"
@@ -14,6 +15,7 @@ struct qft_plan_s {
     QftHostPlan host;
     std::unique_ptr<QftPassCache[]> cache;  // one per pass: encoded tensor maps, kernel attributes (qft_launch.h)
     std::mutex host_mu;                     // serialises qft_execute_host on this plan
+    std::atomic<bool> single_launch{false}; // the whole transform fits the one-launch kernel (qft_launch.h)
     void* dev_buf = nullptr;                // only for qft_execute_host
     int dev_buf_device = -1;
     size_t dev_bytes = 0;
@@ -36,7 +38,10 @@ static qft_status_t create_from(qft_plan_t* out, const QftPlanParams& prm) {
     int rc;
     try {
         rc = qft_build_plan(prm, &p->host, &err);
-        if (rc == 0) p->cache.reset(new QftPassCache[p->host.passes.size()]);
+        if (rc == 0) {
+            p->cache.reset(new QftPassCache[p->host.passes.size()]);
+            p->single_launch = !(prm.flags & QFT_FLAG_MULTI_LAUNCH) && qft_plan_fits_single_launch(p->host);
+        }
     } catch (const std::bad_alloc&) {
         delete p;
         return QFT_ERR_ALLOC;
@@ -88,6 +93,13 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream) {
     if (!plan || !device_state) return QFT_ERR_INVALID_ARG;
     const uintptr_t align = plan->host.prm.n >= 1 ? 16 : 8;
     if (((uintptr_t)device_state) & (align - 1)) return QFT_ERR_INVALID_ARG;
+    if (plan->single_launch.load(std::memory_order_relaxed)) {
+        // small states (n = 20 ... 24): all passes in one cooperative launch with grid-wide barriers between them
+        cudaError_t e = qft_launch_single(plan->host, plan->cache.get(), device_state, (cudaStream_t)stream);
+        if (e == cudaSuccess) return QFT_OK;
+        cudaGetLastError();  // nothing was enqueued: from now on this plan launches its passes one by one
+        plan->single_launch = false;
+    }
     for (size_t i = 0; i < plan->host.passes.size(); ++i) {
         cudaError_t e = qft_launch_pass(plan->host.passes[i], &plan->cache[i], device_state, device_state, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(e);
@@ -173,7 +185,10 @@ qft_status_t qft_plan_destroy(qft_plan_t plan) {
 }
 
 int qft_plan_num_passes(qft_plan_t plan) { return plan ? (int)plan->host.passes.size() : -1; }
-int qft_plan_num_launches(qft_plan_t plan) { return plan ? (int)plan->host.passes.size() : -1; }
+int qft_plan_num_launches(qft_plan_t plan) {
+    if (!plan) return -1;
+    return plan->single_launch.load(std::memory_order_relaxed) ? 1 : (int)plan->host.passes.size();
+}
 
 qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_cr, long long* n_swap) {
     if (!plan || !n_h || !n_cr || !n_swap) return QFT_ERR_INVALID_ARG;

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256, 2) qft_pass_fused2(float2* __restrict__ s
     const int f = d.f;
 
     uint32_t mload, mstore;
-    decode_tile(blockIdx.x, d.npair, &mload, &mstore);
+    decode_tile(blockIdx.x + (uint32_t)d.unit_lo * (d.npair ? 2u : 1u), d.npair, &mload, &mstore);
     uint64_t base_ld = 0, base_st = 0, Ltile = 0;
     for (int i = 0; i < d.ntile; ++i) {
         if ((mload >> i) & 1u) {

@@ -766,7 +766,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         *err = "invalid argument";
         return 1;
     }
-    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u)) { *err = "unknown flag"; return 2; }
+    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u | 64u)) { *err = "unknown flag"; return 2; }
     if ((prm.flags & 32u) && (prm.flags & 2u)) { *err = "deferred swaps have no unfolded schedule"; return 2; }
     // defaults from the B200 sweeps (profiles/r01_tile_hub_sweep.md, profiles/r02_tile_hub_sweep.md): 128-byte
     // granules (hub 4) as soon as the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit

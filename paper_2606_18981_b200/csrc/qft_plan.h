@@ -83,6 +83,9 @@ struct QftPassDesc {
     float scale;        // applied in the last step (1 unless this is the final pass)
     int32_t do_scale;
     int32_t win_lo;     // lowest logical qubit the register steps process (-1: permutation-only pass)
+    // the units (tiles, or pairs of tiles of a pair pass) this launch walks: [unit_lo, unit_lo + unit_n); unit_n = 0:
+    // all of them.  Set per launch by qft_execute_pass_shard (one rank's share of a pass), 0 in the plan.
+    int32_t unit_lo, unit_n;
     // ---- tensor-memory extended tile (QFT_KERNEL_TMA2 only) ------------------------------------
     // xt = 1: the pass owns tiles of 2^(f+1) amplitudes, F + {xt_ld_addr}.  A CTA runs the two halves
     // (address bit xt_ld_addr = 0, then 1) through the register steps one after the other, parks the

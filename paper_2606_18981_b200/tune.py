@@ -26,6 +26,7 @@ def main() -> int:
     ap.add_argument("--log2-batch", type=int, default=0, help="2^b independent transforms back to back")
     ap.add_argument("--reps", type=int, default=2)
     ap.add_argument("--no-time", action="store_true")
+    ap.add_argument("--loop", type=int, default=0, help="also time this many back-to-back qft_execute calls (launch-bound sizes)")
     a = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("needs a CUDA device")
@@ -60,8 +61,19 @@ def main() -> int:
         qft.qft_execute(plan.handle, st.data_ptr(), s)
     e1.record()
     torch.cuda.synchronize()
+    loop_us = None
+    if a.loop:
+        for _ in range(20):
+            qft.qft_execute(plan.handle, st.data_ptr(), s)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(a.loop):
+            qft.qft_execute(plan.handle, st.data_ptr(), s)
+        e1.record()
+        torch.cuda.synchronize()
+        loop_us = round(1000.0 * e0.elapsed_time(e1) / a.loop, 2)
     d = plan.describe()
-    print(json.dumps({"n": d["n"], "batch_bits": d["batch_bits"], "k": d["k"], "tile_bits": d["tile_bits"], "hub_bits": d["hub_bits"], "passes": npass,
+    print(json.dumps({"launches": plan.num_launches, "loop_us_per_execute": loop_us, "n": d["n"], "batch_bits": d["batch_bits"], "k": d["k"], "tile_bits": d["tile_bits"], "hub_bits": d["hub_bits"], "passes": npass,
                       "kernels": [p["kernel"] for p in d["passes"]], "steps": [p["steps"] for p in d["passes"]],
                       "pass_ms": [round(v, 3) for v in acc], "execute_ms": round(e0.elapsed_time(e1) / reps, 3),
                       "gbs_per_pass": [round(16.0 * (1 << n) / v / 1e6) for v in acc]}))

@@ -511,28 +511,26 @@ def main():
     if args.small_n and rank == 0 and world == 1:
         torch.cuda.empty_cache()
         for sn in [int(v) for v in args.small_n.split(",") if v]:
-            row = {"n": sn, "transforms": 1000}
-            for label, fl in (("one_launch", args.flags), ("launch_per_pass", args.flags | qft.QFT_FLAG_MULTI_LAUNCH)):
-                pl = qft.Plan(sn, sn if args.k is None else args.k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
-                              args.hub_bits, fl)
-                stt = torch.empty(1 << sn, dtype=torch.complex64, device="cuda")
-                torch.view_as_real(stt).normal_()
-                stt.mul_(2.0 ** (-(sn + 1) / 2))
-                strm = torch.cuda.current_stream()
-                for _ in range(20):
-                    qft.qft_execute(pl.handle, stt.data_ptr(), strm.cuda_stream)
-                torch.cuda.synchronize()
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(strm)
-                for _ in range(1000):
-                    qft.qft_execute(pl.handle, stt.data_ptr(), strm.cuda_stream)
-                e1.record(strm)
-                torch.cuda.synchronize()
-                us = e0.elapsed_time(e1)  # ms for 1000 transforms = microseconds per transform
-                row[label] = {"us_per_transform": us, "launches": pl.num_launches,
-                              "gflops": 5.0 * (1 << sn) * sn / (us * 1e-6) / 1e9}
-                pl.close()
-                del stt
+            pl = qft.Plan(sn, sn if args.k is None else args.k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
+                          args.hub_bits, args.flags)
+            stt = torch.empty(1 << sn, dtype=torch.complex64, device="cuda")
+            torch.view_as_real(stt).normal_()
+            stt.mul_(2.0 ** (-(sn + 1) / 2))
+            strm = torch.cuda.current_stream()
+            for _ in range(20):
+                qft.qft_execute(pl.handle, stt.data_ptr(), strm.cuda_stream)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(strm)
+            for _ in range(1000):
+                qft.qft_execute(pl.handle, stt.data_ptr(), strm.cuda_stream)
+            e1.record(strm)
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1)  # ms for 1000 transforms = microseconds per transform
+            row = {"n": sn, "transforms": 1000, "us_per_transform": us, "launches_per_transform": pl.num_launches,
+                   "gflops": 5.0 * (1 << sn) * sn / (us * 1e-6) / 1e9}
+            pl.close()
+            del stt
             small.append(row)
 
     # ---- CPU baseline: the oracle as it stands, WHOLE circuits, rank 0 at N = 1 only ----

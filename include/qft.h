@@ -124,12 +124,6 @@ qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_bat
  * the granule size; callers must read it from the plan, not assume it.  Not available for batched plans.
  */
 #define QFT_FLAG_DEFER_SWAPS 32u
-/* QFT_FLAG_MULTI_LAUNCH -- one kernel launch per pass even where the whole transform would run in one.  By default
- * a plan whose state lives in L2 (n = 20 ... 24, the paper's measured sizes: Fig. 4) and whose three
- * passes share a tile size runs as ONE cooperative launch with grid-wide barriers between the passes (no launch gaps,
- * tables of pass p + 1 built while pass p drains).  qft_plan_num_launches reports which applies; if the device refuses
- * the cooperative launch (not enough SMs free for the whole grid) the plan silently reverts to one launch per pass. */
-#define QFT_FLAG_MULTI_LAUNCH 64u
 qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                                    qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
 
@@ -182,6 +176,29 @@ qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_stat
 
 /* qft_plan_destroy -- free the plan and everything it owns.  NULL is allowed. */
 qft_status_t qft_plan_destroy(qft_plan_t plan);
+
+/*
+ * Sharded state, host-side design (PAPER.md:229 outlook "scale with distributed simulators"; not measured on more than
+ * one GPU).  The 2^n amplitudes live on 2^log2_ranks ranks; the top log2_ranks address bits select the rank and the
+ * shards are mapped back to back into ONE virtual address range on every rank (peer memory over NVLink), so every
+ * pass is the same kernel on the same addresses.  Rank r runs its share of the units of pass p,
+ * qft_execute_pass_shard(plan, p, base, r, log2_ranks, stream), all ranks synchronise (a barrier, no data-path
+ * collective), then pass p + 1.  A pass whose tiles hold no rank bit is local (rank r's units touch only its own
+ * shard); a pass whose tiles hold g_in rank bits reads and writes a fraction 1 - 2^-g_in of its bytes on peers:
+ * the all-to-all of the classical scheme, fused into the pass's loads and stores.
+ *   qft_plan_shard_info: rank r's unit range of the pass, the rank bits inside its tiles and the bytes it moves over
+ *     the links in each direction.  QFT_ERR_UNSUPPORTED if a rank bit takes part in a pair involution or the pass has
+ *     fewer units than ranks (qft_last_cuda_error says which).
+ *   qft_plan_shard_check: host proof for every pass and rank that the ranges tile the pass and that a local pass's
+ *     units lie on their own rank (replays the kernel's unit -> tile -> address maps).
+ *   qft_execute_pass_shard: enqueue rank r's share.  With every rank's share enqueued one after the other on ONE
+ *     device (same buffer) the result is exactly qft_execute_pass; that is how the path is tested on one GPU.
+ */
+qft_status_t qft_plan_shard_info(qft_plan_t plan, int pass_index, int rank, int log2_ranks, long long* unit_lo,
+                                 long long* unit_n, int* rank_bits_in_tile, long long* remote_bytes_each_way);
+qft_status_t qft_plan_shard_check(qft_plan_t plan, int log2_ranks);
+qft_status_t qft_execute_pass_shard(qft_plan_t plan, int pass_index, void* state_base, int rank, int log2_ranks,
+                                    void* stream);
 
 /* Introspection (the paper's plan carries the fused blocks and the counters of
  * 1- and 2-qubit gates before fusion). */

@@ -22,7 +22,6 @@ LIB_PATH = os.path.join(_HERE, "libqft.so")
 QFT_OK, QFT_ERR_INVALID_ARG, QFT_ERR_UNSUPPORTED, QFT_ERR_ALLOC, QFT_ERR_CUDA, QFT_ERR_INTERNAL = range(6)
 QFT_NORM_UNITARY, QFT_NORM_NONE, QFT_NORM_INV_N = 0, 1, 2
 QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_NO_EXT_TILE, QFT_FLAG_DEFER_SWAPS = 1, 2, 4, 16, 32
-QFT_FLAG_MULTI_LAUNCH = 64
 QFT_MAX_QUBITS = 34
 
 EXPORTS = [
@@ -30,6 +29,7 @@ EXPORTS = [
     "qft_plan_num_passes", "qft_plan_num_launches", "qft_plan_gate_counts", "qft_plan_describe",
     "qft_plan_describe_length", "qft_num_qubits_for", "qft_encode_padded", "qft_execute_oop", "qft_plan_output_order",
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
+    "qft_plan_shard_info", "qft_plan_shard_check", "qft_execute_pass_shard",
     "qft_norm_sq", "qft_encode", "qft_rescale", "qft_fidelity", "qft_leakage",
 ]
 
@@ -74,6 +74,13 @@ def load() -> ctypes.CDLL:
     L.qft_plan_output_order.restype = ci
     L.qft_execute_pass.argtypes = [vp, ci, vp, vp]
     L.qft_execute_pass.restype = ci
+    L.qft_plan_shard_info.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong),
+                                      ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_longlong)]
+    L.qft_plan_shard_info.restype = ci
+    L.qft_plan_shard_check.argtypes = [vp, ci]
+    L.qft_plan_shard_check.restype = ci
+    L.qft_execute_pass_shard.argtypes = [vp, ci, vp, ci, ci, vp]
+    L.qft_execute_pass_shard.restype = ci
     L.qft_execute_host.argtypes = [vp, vp, vp]
     L.qft_execute_host.restype = ci
     L.qft_plan_destroy.argtypes = [vp]
@@ -175,6 +182,27 @@ def qft_execute_pass(plan: int, pass_index: int, device_state_ptr: int, stream: 
     st = load().qft_execute_pass(plan, pass_index, device_state_ptr, stream)
     if st != QFT_OK:
         raise QftError(st, "qft_execute_pass")
+
+
+def qft_plan_shard_info(plan: int, pass_index: int, rank: int, log2_ranks: int) -> dict:
+    lo, cnt, rem, gin = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_int()
+    st = load().qft_plan_shard_info(plan, pass_index, rank, log2_ranks, ctypes.byref(lo), ctypes.byref(cnt), ctypes.byref(gin),
+                                    ctypes.byref(rem))
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_shard_info")
+    return {"unit_lo": lo.value, "unit_n": cnt.value, "rank_bits_in_tile": gin.value, "remote_bytes_each_way": rem.value}
+
+
+def qft_plan_shard_check(plan: int, log2_ranks: int) -> None:
+    st = load().qft_plan_shard_check(plan, log2_ranks)
+    if st != QFT_OK:
+        raise QftError(st, "qft_plan_shard_check")
+
+
+def qft_execute_pass_shard(plan: int, pass_index: int, state_base_ptr: int, rank: int, log2_ranks: int, stream: int = 0) -> None:
+    st = load().qft_execute_pass_shard(plan, pass_index, state_base_ptr, rank, log2_ranks, stream)
+    if st != QFT_OK:
+        raise QftError(st, "qft_execute_pass_shard")
 
 
 def qft_execute_host(plan: int, host_state_ptr: int, stream: int = 0) -> None:

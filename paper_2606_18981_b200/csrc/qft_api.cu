@@ -5,7 +5,6 @@
 #include <new>
 #include <string>
 
-#include <atomic>
 #include <memory>
 
 #include "../../include/qft.h"
@@ -15,7 +14,6 @@ struct qft_plan_s {
     QftHostPlan host;
     std::unique_ptr<QftPassCache[]> cache;  // one per pass: encoded tensor maps, kernel attributes (qft_launch.h)
     std::mutex host_mu;                     // serialises qft_execute_host on this plan
-    std::atomic<bool> single_launch{false}; // the whole transform fits the one-launch kernel (qft_launch.h)
     void* dev_buf = nullptr;                // only for qft_execute_host
     int dev_buf_device = -1;
     size_t dev_bytes = 0;
@@ -38,10 +36,7 @@ static qft_status_t create_from(qft_plan_t* out, const QftPlanParams& prm) {
     int rc;
     try {
         rc = qft_build_plan(prm, &p->host, &err);
-        if (rc == 0) {
-            p->cache.reset(new QftPassCache[p->host.passes.size()]);
-            p->single_launch = !(prm.flags & QFT_FLAG_MULTI_LAUNCH) && qft_plan_fits_single_launch(p->host);
-        }
+        if (rc == 0) p->cache.reset(new QftPassCache[p->host.passes.size()]);
     } catch (const std::bad_alloc&) {
         delete p;
         return QFT_ERR_ALLOC;
@@ -93,13 +88,6 @@ qft_status_t qft_execute(qft_plan_t plan, void* device_state, void* stream) {
     if (!plan || !device_state) return QFT_ERR_INVALID_ARG;
     const uintptr_t align = plan->host.prm.n >= 1 ? 16 : 8;
     if (((uintptr_t)device_state) & (align - 1)) return QFT_ERR_INVALID_ARG;
-    if (plan->single_launch.load(std::memory_order_relaxed)) {
-        // small states (n = 20 ... 24): all passes in one cooperative launch with grid-wide barriers between them
-        cudaError_t e = qft_launch_single(plan->host, plan->cache.get(), device_state, (cudaStream_t)stream);
-        if (e == cudaSuccess) return QFT_OK;
-        cudaGetLastError();  // nothing was enqueued: from now on this plan launches its passes one by one
-        plan->single_launch = false;
-    }
     for (size_t i = 0; i < plan->host.passes.size(); ++i) {
         cudaError_t e = qft_launch_pass(plan->host.passes[i], &plan->cache[i], device_state, device_state, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(e);
@@ -147,6 +135,54 @@ qft_status_t qft_execute_pass(qft_plan_t plan, int pass_index, void* device_stat
     return QFT_OK;
 }
 
+qft_status_t qft_plan_shard_info(qft_plan_t plan, int pass_index, int rank, int log2_ranks, long long* unit_lo,
+                                 long long* unit_n, int* rank_bits_in_tile, long long* remote_bytes_each_way) {
+    if (!plan || pass_index < 0 || pass_index >= (int)plan->host.passes.size() || !unit_lo || !unit_n || !rank_bits_in_tile ||
+        !remote_bytes_each_way)
+        return QFT_ERR_INVALID_ARG;
+    std::string err;
+    const int rc = qft_shard_range(plan->host, (size_t)pass_index, rank, log2_ranks, unit_lo, unit_n, rank_bits_in_tile, &err);
+    if (rc != 0) {
+        g_cuda_err = err;
+        return (qft_status_t)rc;
+    }
+    const QftPassDesc& d = plan->host.passes[pass_index];
+    const long long bytes = (*unit_n * (d.npair ? 2 : 1)) * ((long long)8 << (d.f + d.xt));  // this rank's share of the pass
+    *remote_bytes_each_way = bytes - (bytes >> *rank_bits_in_tile);
+    return QFT_OK;
+}
+
+qft_status_t qft_plan_shard_check(qft_plan_t plan, int log2_ranks) {
+    if (!plan) return QFT_ERR_INVALID_ARG;
+    std::string err;
+    const int rc = qft_check_shard(plan->host, log2_ranks, &err);
+    if (rc != 0) {
+        g_cuda_err = err;
+        return (qft_status_t)rc;
+    }
+    return QFT_OK;
+}
+
+qft_status_t qft_execute_pass_shard(qft_plan_t plan, int pass_index, void* state_base, int rank, int log2_ranks,
+                                    void* stream) {
+    if (!plan || !state_base || pass_index < 0 || pass_index >= (int)plan->host.passes.size()) return QFT_ERR_INVALID_ARG;
+    if (((uintptr_t)state_base) & 15) return QFT_ERR_INVALID_ARG;
+    long long lo, cnt;
+    int g_in;
+    std::string err;
+    const int rc = qft_shard_range(plan->host, (size_t)pass_index, rank, log2_ranks, &lo, &cnt, &g_in, &err);
+    if (rc != 0) {
+        g_cuda_err = err;
+        return (qft_status_t)rc;
+    }
+    QftPassDesc d = plan->host.passes[pass_index];
+    d.unit_lo = (int32_t)lo;
+    d.unit_n = (int32_t)cnt;
+    cudaError_t e = qft_launch_pass(d, &plan->cache[pass_index], state_base, state_base, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return QFT_OK;
+}
+
 qft_status_t qft_execute_host(qft_plan_t plan, void* host_state, void* stream) {
     if (!plan || !host_state) return QFT_ERR_INVALID_ARG;
     const size_t bytes = (size_t)8 << (plan->host.prm.n + plan->host.prm.batch_bits);
@@ -185,10 +221,7 @@ qft_status_t qft_plan_destroy(qft_plan_t plan) {
 }
 
 int qft_plan_num_passes(qft_plan_t plan) { return plan ? (int)plan->host.passes.size() : -1; }
-int qft_plan_num_launches(qft_plan_t plan) {
-    if (!plan) return -1;
-    return plan->single_launch.load(std::memory_order_relaxed) ? 1 : (int)plan->host.passes.size();
-}
+int qft_plan_num_launches(qft_plan_t plan) { return plan ? (int)plan->host.passes.size() : -1; }
 
 qft_status_t qft_plan_gate_counts(qft_plan_t plan, long long* n_h, long long* n_cr, long long* n_swap) {
     if (!plan || !n_h || !n_cr || !n_swap) return QFT_ERR_INVALID_ARG;

@@ -19,9 +19,6 @@
 #include "qft_launch.h"
 
 #include <algorithm>
-#include <atomic>
-#include <utility>
-#include <vector>
 
 namespace qftk {
 
@@ -378,103 +375,6 @@ static cudaError_t launch_tma2(const QftPassDesc& d_in, QftPassCache* cache, int
     attr[cfg.numAttrs].val.programmaticStreamSerializationAllowed = 1;
     ++cfg.numAttrs;
     void* args[3] = {(void*)&state, (void*)&map, (void*)&d};
-    return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
-}
-
-// ---- the whole transform in one launch (qft_multi_tma2) -------------------------------------------------------
-typedef void (*tma2_multi_kernel_t)(float2*, const CUtensorMap, const CUtensorMap, const CUtensorMap, const QftPassDesc,
-                                    const QftPassDesc, const QftPassDesc, unsigned*);
-tma2_multi_kernel_t qft_pick_tma2_multi7(int a1, int a2, int b1, int b2, int kc);  // qft_tma_multi7.cu
-tma2_multi_kernel_t qft_pick_tma2_multi8(int a1, int a2, int b1, int b2, int kc);  // qft_tma_multi8.cu
-
-// barrier slots of the single-launch kernel: (arrival count, generation) pairs, zero when the module is loaded and
-// left at count 0 by every launch; a launch takes the next slot round robin
-__device__ unsigned g_qft_grid_barrier[2 * 256];
-static std::atomic<unsigned> g_next_slot{0};
-
-static tma2_multi_kernel_t pick_multi(const QftPassDesc* p) {
-    const int kc = p[0].k < 4 ? p[0].k : 4;
-    const int lt = p[0].log2_threads;
-    if (lt == 7) return qft_pick_tma2_multi7(p[0].tma.r1, p[0].tma.r2, p[1].tma.r1, p[1].tma.r2, kc);
-    if (lt == 8) return qft_pick_tma2_multi8(p[0].tma.r1, p[0].tma.r2, p[1].tma.r1, p[1].tma.r2, kc);
-    return nullptr;
-}
-
-// Plans the single-launch kernel can run: three TMA-staged passes on the same tile size, the outer two with the same
-// register-group shape, no extended tile, no split end table, and a state small enough to live in L2 (n <= 24).
-bool qft_plan_fits_single_launch(const QftHostPlan& plan) {
-    if (plan.passes.size() != 3 || plan.prm.batch_bits != 0 || plan.prm.n > 24) return false;
-    const QftPassDesc* p = plan.passes.data();
-    for (int i = 0; i < 3; ++i)
-        if (p[i].kernel != QFT_KERNEL_TMA2 || p[i].xt || p[i].tma.eb > QFT_TMA2_EB_DIRECT || p[i].f != p[0].f) return false;
-    if (p[0].tma.r1 != p[2].tma.r1 || p[0].tma.r2 != p[2].tma.r2) return false;
-    return pick_multi(p) != nullptr;
-}
-
-cudaError_t qft_launch_single(const QftHostPlan& plan, QftPassCache* caches, void* state, cudaStream_t stream) {
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    QftPassDesc d[3];
-    CUtensorMap map[3];
-    size_t smem = 0;
-    unsigned long long units = 0;
-    bool pair = false;
-    for (int i = 0; i < 3; ++i) {
-        d[i] = plan.passes[i];
-        fill_units(&d[i]);
-        smem = std::max(smem, ((size_t)8 << d[i].f) + QFT_TMA2_TABLE_BYTES(d[i].tma.eb, d[i].ntile));
-        units = std::max(units, (unsigned long long)d[i].unit_n * (d[i].npair ? 2u : 1u));
-        pair = pair || d[i].npair > 0;
-        std::lock_guard<std::mutex> lock(caches[i].mu);
-        if (!get_map(d[i], &caches[i], dev, state, &map[i])) return cudaErrorNotSupported;
-    }
-    tma2_multi_kernel_t kern = pick_multi(d);
-    if (!kern) return cudaErrorNotSupported;
-    static std::mutex mu;
-    static unsigned* slots[64];
-    static std::vector<std::pair<int, const void*>> attr_done;  // (device, kernel) pairs whose shared-memory limit is set
-    unsigned* base = nullptr;
-    {
-        std::lock_guard<std::mutex> lock(mu);
-        if (dev < 0 || dev >= 64) return cudaErrorNotSupported;
-        if (!slots[dev]) {
-            e = cudaGetSymbolAddress((void**)&slots[dev], g_qft_grid_barrier);
-            if (e != cudaSuccess) return e;
-        }
-        base = slots[dev];
-        const std::pair<int, const void*> key(dev, (const void*)kern);
-        if (std::find(attr_done.begin(), attr_done.end(), key) == attr_done.end()) {
-            e = cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin(dev));
-            if (e != cudaSuccess) return e;
-            attr_done.push_back(key);
-        }
-    }
-    // every CTA must be resident: one wave at most
-    unsigned long long grid = (unsigned long long)sm_count(dev) * tma2_ctas_per_sm(d[0], smem);
-    if (grid > units) grid = units;
-    grid -= grid % 2;
-    if (grid < 2) return cudaErrorNotSupported;
-    unsigned* slot = base + 2 * (g_next_slot.fetch_add(1) % 256u);
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(1u << d[0].log2_threads);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[2];
-    cfg.attrs = attr;
-    cfg.numAttrs = 0;
-    if (pair) {
-        attr[cfg.numAttrs].id = cudaLaunchAttributeClusterDimension;
-        attr[cfg.numAttrs].val.clusterDim.x = 2;
-        attr[cfg.numAttrs].val.clusterDim.y = 1;
-        attr[cfg.numAttrs].val.clusterDim.z = 1;
-        ++cfg.numAttrs;
-    }
-    attr[cfg.numAttrs].id = cudaLaunchAttributeCooperative;
-    attr[cfg.numAttrs].val.cooperative = 1;
-    ++cfg.numAttrs;
-    void* args[8] = {(void*)&state, (void*)&map[0], (void*)&map[1], (void*)&map[2], (void*)&d[0], (void*)&d[1], (void*)&d[2], (void*)&slot};
     return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
 }
 

@@ -25,9 +25,3 @@ struct QftPassCache {
 // different one only if qft_pass_reads_through_tensor_map(d), else cudaErrorNotSupported).
 cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* src, void* state, cudaStream_t stream);
 bool qft_pass_reads_through_tensor_map(const QftPassDesc& d);
-
-// The whole transform in one cooperative launch (plans with qft_plan_fits_single_launch): caches = the plan's per-pass
-// caches.  An error (e.g. the device cannot hold the grid at once) leaves nothing enqueued; the caller then launches
-// the passes one by one.
-bool qft_plan_fits_single_launch(const QftHostPlan& plan);
-cudaError_t qft_launch_single(const QftHostPlan& plan, QftPassCache* caches, void* state, cudaStream_t stream);

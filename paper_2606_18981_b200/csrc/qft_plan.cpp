@@ -766,12 +766,15 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         *err = "invalid argument";
         return 1;
     }
-    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u | 64u)) { *err = "unknown flag"; return 2; }
+    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u)) { *err = "unknown flag"; return 2; }
     if ((prm.flags & 32u) && (prm.flags & 2u)) { *err = "deferred swaps have no unfolded schedule"; return 2; }
     // defaults from the B200 sweeps (profiles/r01_tile_hub_sweep.md, profiles/r02_tile_hub_sweep.md): 128-byte
     // granules (hub 4) as soon as the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit
     // windows pay off (n = 13: three multi-CTA passes on 2^12 tiles take 17 us, one 8192-amplitude CTA takes 30 us)
-    int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : (n == 13 && prm.batch_bits == 0 ? 12 : 13));
+    // (n = 20 ... 23, state resident in L2: 2^12 tiles put twice as many CTAs in flight, 19 vs 21.5 us at n = 20, 37.8 vs
+    // 42.4 us at n = 22: profiles/r02_small_n.md)
+    int fmax = prm.tile_bits ? prm.tile_bits
+                             : (n >= 26 ? 14 : (prm.batch_bits == 0 && (n == 13 || (n >= 20 && n <= 23)) ? 12 : 13));
     // 256-byte granules (hub 5) where a 10-qubit window still gives the minimum number of passes: with the
     // tensor-memory extension that is n = 26 ... 30 (3 passes) and n = 34 (4 passes); n = 31 ... 33 need 11-qubit
     // windows for 3 passes, i.e. 128-byte granules (profiles/r02_tile_hub_sweep.md)
@@ -1155,6 +1158,92 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
     }
     const bool want_scale = plan.prm.norm != 1;
     if ((want_scale && nscaled != 1) || (!want_scale && nscaled != 0)) { *err = "self-check: scale"; return 5; }
+    return 0;
+}
+
+// Sharded state (host-side design): the 2^n amplitudes
+// live on 2^g ranks, the top g address bits select the rank, and the shards are mapped back to back into one virtual
+// range (peer memory over NVLink), so a pass is the same kernel on the same addresses and only the question "which
+// rank runs which units" is new.  A rank bit is either a tile-index bit (the units whose value of that bit equals
+// the rank's touch only that rank's shard: local) or a tile bit (every unit's rows lie on both values: spanning).
+// Rank bits outside the tile are always the top bits of the unit index (they are the highest non-tile addresses), so
+// a rank's share is one contiguous unit range: the units whose outside rank bits equal its own, split evenly among
+// the 2^g_in ranks that share them.  Unsupported: a rank bit inside a pair involution (the folded schedule never
+// does that for g <= hub bits), fewer units than ranks.
+// Returns 0, or 2 (unsupported) with *err set.
+int qft_shard_range(const QftHostPlan& plan, size_t pass, int rank, int g, long long* unit_lo, long long* unit_n,
+                    int* rank_bits_in_tile, std::string* err) {
+    const QftPassDesc& d = plan.passes[pass];
+    const int n = d.n;
+    if (g < 0 || g > 6 || g >= n || rank < 0 || rank >= (1 << g)) { *err = "invalid rank / log2_ranks"; return 1; }
+    std::vector<int> inTile(n, 0), inPair(n, 0);
+    for (int j = 0; j < d.f; ++j) inTile[d.F[j]] = 1;
+    if (d.xt) inTile[d.xt_ld_addr] = 1;
+    for (int i = 0; i < 2 * d.npair; ++i) inPair[d.tile_addr[i]] = 1;
+    int g_in = 0;
+    unsigned o = 0, r_in = 0;
+    int m = 0;
+    for (int b = 0; b < g; ++b) {
+        const int a = n - g + b;
+        const unsigned bit = ((unsigned)rank >> b) & 1u;
+        if (inPair[a]) { *err = "a rank bit trades places with another address bit in this pass"; return 2; }
+        if (inTile[a]) r_in |= bit << g_in++;
+        else o |= bit << m++;
+    }
+    const int ubits = d.ntile - d.xt - (d.npair ? 1 : 0);  // log2 of the number of units
+    if (ubits < g) { *err = "fewer units than ranks"; return 2; }
+    const long long per_o = 1ll << (ubits - m);  // units that share one value of the outside rank bits
+    *unit_n = per_o >> g_in;
+    *unit_lo = (long long)o * per_o + (long long)r_in * *unit_n;
+    *rank_bits_in_tile = g_in;
+    return 0;
+}
+
+// Host proof of the sharding rule for every pass and rank: the ranges tile the unit space exactly, and every unit of
+// rank r's range has the outside rank bits of r (replayed through the kernel's own unit -> tile -> address maps).
+int qft_check_shard(const QftHostPlan& plan, int g, std::string* err) {
+    char buf[160];
+    for (size_t p = 0; p < plan.passes.size(); ++p) {
+        const QftPassDesc& d = plan.passes[p];
+        const int n = d.n;
+        const int ubits = d.ntile - d.xt - (d.npair ? 1 : 0);
+        std::vector<std::pair<long long, long long>> ranges;
+        for (int r = 0; r < (1 << g); ++r) {
+            long long lo, cnt;
+            int g_in;
+            const int rc = qft_shard_range(plan, p, r, g, &lo, &cnt, &g_in, err);
+            if (rc != 0) return rc;
+            ranges.push_back({lo, cnt});
+            // first and last unit of the range, and one in the middle: tile-index value -> address bits
+            for (long long u : {lo, lo + cnt / 2, lo + cnt - 1}) {
+                // unit -> tile index of the unit's first CTA: without pairs the unit itself; with p pairs the
+                // cluster id, whose bits above 2p - 1 are the tile-index bits above the pairs
+                unsigned long long tile_hi = d.npair ? ((unsigned long long)u >> (2 * d.npair - 1)) << (2 * d.npair) : (unsigned long long)u;
+                for (int b = 0; b < g; ++b) {
+                    const int a = n - g + b;
+                    bool in_tile = d.xt && a == d.xt_ld_addr;
+                    for (int j = 0; j < d.f; ++j) in_tile = in_tile || d.F[j] == a;
+                    if (in_tile) continue;
+                    int idx = -1;
+                    for (int i = 0; i < d.ntile - d.xt; ++i)
+                        if (d.tile_addr[i] == a) idx = i;
+                    if (idx < 0) { *err = "shard check: rank bit is neither a tile nor a tile-index bit"; return 5; }
+                    if (((tile_hi >> idx) & 1ull) != (((unsigned)r >> b) & 1u)) {
+                        snprintf(buf, sizeof buf, "shard check: pass %zu rank %d: unit %lld lies on another rank", p, r, u);
+                        *err = buf;
+                        return 5;
+                    }
+                }
+            }
+        }
+        std::sort(ranges.begin(), ranges.end());
+        long long next = 0;
+        for (auto& rg : ranges) {
+            if (rg.first != next || rg.second < 1) { *err = "shard check: unit ranges do not tile the pass"; return 5; }
+            next += rg.second;
+        }
+        if (next != (1ll << ubits)) { *err = "shard check: unit ranges do not cover the pass"; return 5; }
+    }
     return 0;
 }
 

@@ -149,3 +149,8 @@ struct QftHostPlan {
 int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err);
 int qft_check_plan(const QftHostPlan& plan, std::string* err);
 std::string qft_describe_plan(const QftHostPlan& plan);
+
+// sharded state, host side (qft_plan.cpp): rank r's unit range of a pass, and the proof that the ranges tile the pass
+int qft_shard_range(const QftHostPlan& plan, size_t pass, int rank, int log2_ranks, long long* unit_lo, long long* unit_n,
+                    int* rank_bits_in_tile, std::string* err);
+int qft_check_shard(const QftHostPlan& plan, int log2_ranks, std::string* err);

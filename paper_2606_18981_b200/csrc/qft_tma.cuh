@@ -176,52 +176,15 @@ struct BatchApply {
 #define QFT_PHASE(i)
 #endif
 
-// ---- grid-wide barrier of the single-launch kernel (qft_multi_tma2) ----------------------------------
-// slot[0] counts arrivals, slot[1] is the generation.  The last CTA to arrive resets the count and bumps the
-// generation; everybody else waits for the generation to change.  Split phase: a CTA arrives when its stores of
-// pass p are done, builds the tables of pass p + 1, and only then waits.  The barrier leaves the slot as it
-// found it (count 0), so a launch needs no host-side reset and can be replayed from a CUDA graph.
-__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ unsigned gbar_arrive(unsigned* slot, unsigned nblocks) {
-    const unsigned gen = ld_acquire_gpu(slot + 1);  // cannot advance before this CTA has arrived
-    unsigned old;
-    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(slot) : "memory");
-    if (old == nblocks - 1u) {
-        asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(slot), "r"(0u) : "memory");
-        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(slot + 1) : "memory");
-    }
-    return gen;
-}
-__device__ __forceinline__ void gbar_wait(const unsigned* slot, unsigned gen) {
-    while (ld_acquire_gpu(slot + 1) == gen) {}
-}
-
 // What a pass waits for before it first touches the state: the previous kernel of the stream (programmatic
-// dependent launch), or the other CTAs' stores of the previous pass of the same launch.
+// dependent launch).  (A functor so that another way of ordering passes can be plugged in: round 2 tried all three
+// passes of an L2-resident state in one cooperative launch with grid-wide barriers here; it was slower than
+// kernel boundaries with programmatic dependent launch, profiles/r02_small_n.md.)
 struct SyncPrevKernel {
     __device__ __forceinline__ void operator()(uint32_t) const { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 };
-struct SyncPrevPass {
-    const unsigned* slot;
-    unsigned gen;
-    bool first;  // the launch's first pass has no predecessor inside the launch
-    __device__ __forceinline__ void operator()(uint32_t tid) const {
-        if (first) return;
-        if (tid == 0) {
-            gbar_wait(slot, gen);
-            asm volatile("fence.proxy.async;" ::: "memory");  // the stores were generic-proxy writes, the loads are TMA's
-        }
-        __syncthreads();
-    }
-};
-
-// One pass over the tiles [d.unit_lo, d.unit_lo + d.unit_n) (all of them when unit_n = 0).  The mbarrier behind the
-// tile lives at a fixed place for a given LT and must have been initialised by the caller; parity carries its
-// phase from one pass of a launch to the next.
+// One pass over the units [d.unit_lo, d.unit_lo + d.unit_n) (the launcher fills the range in: all of them, or one rank's
+// share).  The mbarrier behind the tile must have been initialised by the caller; parity carries its phase.
 template <int R1, int R2, int KC, int LT, int XT, int ES, typename Sync>
 __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUtensorMap* tmap_p, const QftPassDesc& d,
                                           unsigned char* smem_raw, uint32_t& parity, const Sync sync_before_state) {
@@ -591,40 +554,6 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     }
     uint32_t parity = 0;
     tma2_pass<R1, R2, KC, LT, XT, ES>(state, &tmap, d, smem_raw, parity, SyncPrevKernel{});
-}
-
-// The whole transform in ONE launch, for states that live in L2 (n = 20 ... 24, PAPER.md:197's sizes): three passes
-// separated by grid-wide barriers instead of kernel boundaries.  All CTAs must be resident at once (cooperative
-// launch); passes 1 and 3 have the same register-group shape (A1 + A2), the mid pass B1 + B2.
-template <int A1, int A2, int B1, int B2, int KC, int LT>
-__global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
-    qft_multi_tma2(float2* __restrict__ state, const __grid_constant__ CUtensorMap m0, const __grid_constant__ CUtensorMap m1,
-                   const __grid_constant__ CUtensorMap m2, const __grid_constant__ QftPassDesc d0,
-                   const __grid_constant__ QftPassDesc d1, const __grid_constant__ QftPassDesc d2, unsigned* gbar) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    if (threadIdx.x == 0) {
-        mbar_init(tma2_mbar<LT>(smem_raw), 1);
-        fence_proxy_async();
-    }
-    uint32_t parity = 0;
-    unsigned gen = 0;
-#pragma unroll 1
-    for (int p = 0; p < 3; ++p) {
-        if (p == 1) {
-            tma2_pass<B1, B2, KC, LT, 0, 0>(state, &m1, d1, smem_raw, parity, SyncPrevPass{gbar, gen, false});
-        } else {
-            const QftPassDesc& d = p == 0 ? d0 : d2;
-            const CUtensorMap* m = p == 0 ? &m0 : &m2;
-            tma2_pass<A1, A2, KC, LT, 0, 0>(state, m, d, smem_raw, parity, SyncPrevPass{gbar, gen, p == 0});
-        }
-        if (p < 2) {
-            // this thread's stores of pass p: visible to the whole GPU, and ordered before the next pass's TMA loads
-            asm volatile("fence.proxy.async;" ::: "memory");
-            __threadfence();
-            __syncthreads();  // also: every warp is done with this pass's tables before the next pass rewrites them
-            if (threadIdx.x == 0) gen = gbar_arrive(gbar, gridDim.x);
-        }
-    }
 }
 
 }  // namespace qftk

@@ -200,39 +200,3 @@ def test_small_windows_against_oracle(n, tile_bits, w):
     if w <= 4:
         assert deepest > 7, "this configuration was chosen to exercise the split end table"
 
-
-# n = 20 ... 24: the default plan runs its three passes as ONE cooperative launch with grid-wide barriers between them
-# (qft_multi_tma2).  Against the oracle, against the same plan launched pass by pass (same arithmetic: bit for bit),
-# and many times back to back (a barrier or visibility race between passes shows up as a mismatch).
-@pytest.mark.parametrize("n,tile_bits", [(20, 0), (20, 12), (21, 0), (22, 0), (22, 12), (23, 0), (24, 0)])
-def test_single_launch_against_oracle_and_per_pass_launches(n, tile_bits):
-    import torch
-
-    import paper_2606_18981_b200 as qft
-
-    x = qi.gaussian(n, 200 + n)
-    for k, sign, norm in [(None, -1, 0), (3, 1, 1), (0, -1, 0), (9, -1, 2)]:
-        kk = n if k is None else k
-        one = qft.Plan(n, kk, 13, sign, norm, tile_bits, 0, 0)
-        per_pass = qft.Plan(n, kk, 13, sign, norm, tile_bits, 0, qft.QFT_FLAG_MULTI_LAUNCH)
-        assert one.num_launches == 1 and per_pass.num_launches == one.num_passes == 3
-        t = torch.from_numpy(x).cuda()
-        one.execute(t)
-        u = torch.from_numpy(x).cuda()
-        per_pass.execute(u)
-        torch.cuda.synchronize()
-        assert one.num_launches == 1, "the cooperative launch was refused and the plan fell back"
-        assert torch.equal(torch.view_as_real(t), torch.view_as_real(u))
-        assert_parity_numpy(t.cpu().numpy().astype(np.complex128), oracle.qft(x, kk, sign, norm), n, (n, tile_bits, kk, sign, norm))
-        if k is None:
-            # 300 transforms back to back on the same buffer, alternating with nothing in between
-            a = torch.from_numpy(x).cuda()
-            b = torch.from_numpy(x).cuda()
-            for _ in range(300):
-                one.execute(a)
-            for _ in range(300):
-                per_pass.execute(b)
-            torch.cuda.synchronize()
-            assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
-        one.close()
-        per_pass.close()

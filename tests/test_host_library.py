@@ -112,12 +112,8 @@ def test_pass_counts_at_the_bench_configs():
     for n, passes in want.items():
         p = qft.Plan(n, n)
         assert p.num_passes == passes, n
-        # n = 20 ... 24: the three passes run in one cooperative launch (QFT_FLAG_MULTI_LAUNCH turns that off)
-        assert p.num_launches == (1 if 20 <= n <= 24 else passes)
+        assert p.num_launches == passes
         p.close()
-    p = qft.Plan(20, 20, flags=qft.QFT_FLAG_MULTI_LAUNCH)
-    assert (p.num_passes, p.num_launches) == (3, 3)
-    p.close()
     # config 3: sweep of max_fused_qubits at n = 26
     # (ceil(26 / w) passes, every one of them in the TMA-staged kernel: small windows are sub-passes of the folded
     # schedule's windows, not the natural-order schedule with its stand-alone reversal)

@@ -1,0 +1,75 @@
+"""Sharded state, host-side design: the top g address bits select the rank.
+
+CPU: for g = 1, 2, 3 and every n the default plan (and the deferred-swaps plan) passes the host proof
+(qft_plan_shard_check): per pass the ranks' unit ranges tile the pass, local passes keep every rank on its own shard;
+the folded schedule has exactly two passes whose tiles span the ranks (first and last), the mid passes are local, and
+the bytes over the links are (1 - 2^-g) of a shard each way for those two.
+GPU (one device, no kernel waits on another): every rank's share of every pass enqueued one after the other on the same
+buffer must give exactly what qft_execute gives, and the oracle's result.
+"""
+import numpy as np
+import pytest
+
+import paper_2606_18981_b200 as qft
+
+
+@pytest.mark.parametrize("g", [1, 2, 3])
+def test_shard_ranges_pass_the_host_proof(g):
+    for n in list(range(18, 35)):
+        for flags in (0, qft.QFT_FLAG_DEFER_SWAPS):
+            p = qft.Plan(n, n, flags=flags)
+            qft.qft_plan_shard_check(p.handle, g)
+            shard_bytes = 8 << (n - g)
+            spanning = 0
+            for ps in range(p.num_passes):
+                infos = [qft.qft_plan_shard_info(p.handle, ps, r, g) for r in range(1 << g)]
+                gin = infos[0]["rank_bits_in_tile"]
+                assert all(i["rank_bits_in_tile"] == gin for i in infos)
+                for i in infos:
+                    assert i["remote_bytes_each_way"] == shard_bytes - (shard_bytes >> gin)
+                spanning += gin > 0
+            if flags == 0 and p.num_passes == 3 and n >= 28:
+                # first and last pass hold the top address bits, the mid pass is local (at smaller n the mid pass's
+                # tile takes every free address bit as a passive extra, the top ones included)
+                assert spanning == 2, (n, g)
+            p.close()
+
+
+def test_shard_unsupported_cases():
+    p = qft.Plan(12, 12)  # one tile: fewer units than ranks
+    with pytest.raises(qft.QftError) as e:
+        qft.qft_plan_shard_info(p.handle, 0, 0, 1)
+    assert e.value.status == qft.QFT_ERR_UNSUPPORTED
+    with pytest.raises(qft.QftError) as e:
+        qft.qft_plan_shard_info(p.handle, 0, 2, 1)  # rank out of range
+    assert e.value.status == qft.QFT_ERR_INVALID_ARG
+    p.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,g,flags,k", [(20, 1, 0, None), (22, 3, 0, None), (24, 2, 0, 5), (25, 3, 0, None),
+                                         (26, 3, 0, None), (26, 2, 32, None), (21, 2, 0, 0)])
+def test_ranks_shares_one_after_the_other_equal_the_whole_pass(n, g, flags, k):
+    import torch
+
+    import oracle
+    import qft_inputs as qi
+    from parity_bounds import assert_parity_numpy
+
+    x = qi.gaussian(n, 300 + n)
+    kk = n if k is None else k
+    plan = qft.Plan(n, kk, flags=flags)
+    whole = torch.from_numpy(x).cuda()
+    plan.execute(whole)
+    parts = torch.from_numpy(x).cuda()
+    s = torch.cuda.current_stream().cuda_stream
+    order = list(range(1 << g))
+    for ps in range(plan.num_passes):
+        order = order[1:] + order[:1]  # any order of the ranks within a pass
+        for r in order:
+            qft.qft_execute_pass_shard(plan.handle, ps, parts.data_ptr(), r, g, s)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(whole), torch.view_as_real(parts))
+    if flags == 0 and n <= 24:
+        assert_parity_numpy(parts.cpu().numpy().astype(np.complex128), oracle.qft(x, kk), n, (n, g, kk))
+    plan.close()

@@ -771,14 +771,14 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     // defaults from the B200 sweeps (profiles/r01_tile_hub_sweep.md, profiles/r02_tile_hub_sweep.md): 128-byte
     // granules (hub 4) as soon as the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit
     // windows pay off (n = 13: three multi-CTA passes on 2^12 tiles take 17 us, one 8192-amplitude CTA takes 30 us)
-    // (n = 20 ... 23, state resident in L2: 2^12 tiles put twice as many CTAs in flight, 19 vs 21.5 us at n = 20, 37.8 vs
-    // 42.4 us at n = 22: profiles/r02_small_n.md)
-    int fmax = prm.tile_bits ? prm.tile_bits
-                             : (n >= 26 ? 14 : (prm.batch_bits == 0 && (n == 13 || (n >= 20 && n <= 23)) ? 12 : 13));
+    // (n = 13 ... 23, state resident in L2: 2^12 tiles put twice as many CTAs in flight, 19 vs 21.5 us at n = 20, 37.8 vs
+    // 42.4 us at n = 22; with 128-byte granules from n = 14 on the mid pass fits the TMA kernel too, 13.1 vs 18.5 us
+    // at n = 15, 15.4 vs 20.8 us at n = 18: profiles/r02_small_n.md)
+    int fmax = prm.tile_bits ? prm.tile_bits : (n >= 26 ? 14 : (prm.batch_bits == 0 && n >= 13 && n <= 23 ? 12 : 13));
     // 256-byte granules (hub 5) where a 10-qubit window still gives the minimum number of passes: with the
     // tensor-memory extension that is n = 26 ... 30 (3 passes) and n = 34 (4 passes); n = 31 ... 33 need 11-qubit
     // windows for 3 passes, i.e. 128-byte granules (profiles/r02_tile_hub_sweep.md)
-    int l = prm.hub_bits ? prm.hub_bits : (na >= 20 ? 4 : 3);
+    int l = prm.hub_bits ? prm.hub_bits : (na >= 20 || (prm.batch_bits == 0 && n >= 14) ? 4 : 3);
     if (!prm.hub_bits && prm.batch_bits == 0 && fmax == 14 && !(prm.flags & (1u | 2u | 4u | 16u)) && ((n >= 26 && n <= 30) || n == 34))
         l = 5;
     if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 6 || l >= fmax) {

@@ -73,11 +73,14 @@ typedef enum {
  *                     pass applies (the planner's analogue of qsim's
  *                     max_fused_size).  Values above the device
  *                     limit are clamped, not an error: a transform that fits one
- *                     shared-memory tile (n <= 13) is one pass; otherwise a tile holds
- *                     2^14 amplitudes (2^15 with the tensor-memory extension, n >= 26),
- *                     of which 4 or 5 address bits are the contiguous granule, so a
- *                     pass processes up to 10 or 11 qubits.  The result does not
- *                     depend on it, only the number of passes does.
+ *                     shared-memory tile (n <= 12) is one pass; otherwise a tile holds
+ *                     2^12 (n = 13 ... 23), 2^13 (n = 24, 25) or 2^14 amplitudes (n >= 26;
+ *                     2^15 with the tensor-memory extension), of which 3 to 6 address bits
+ *                     are the contiguous granule, so a pass processes up to 8 ... 11 qubits
+ *                     (n = 30: three passes of 10, n = 33: three of 11).  Values of 6 and
+ *                     below cut those windows into sub-passes of at most that many qubits
+ *                     (n = 26: 13 / 7 / 5 passes for 2 / 4 / 6).  The result does not depend
+ *                     on it, only the number of passes does.
  *   sign              -1: the paper's forward transform; +1: every phase
  *                     conjugated.  With unitary normalisation this is the exact
  *                     inverse of the sign = -1 transform with the same k, for every

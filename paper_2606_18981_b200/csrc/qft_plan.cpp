@@ -780,7 +780,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     // windows for 3 passes, i.e. 128-byte granules (profiles/r02_tile_hub_sweep.md)
     int l = prm.hub_bits ? prm.hub_bits : (na >= 20 || (prm.batch_bits == 0 && n >= 14) ? 4 : 3);
     if (!prm.hub_bits && prm.batch_bits == 0 && fmax == 14 && !(prm.flags & (1u | 2u | 4u | 16u)) && ((n >= 26 && n <= 30) || n == 34))
-        l = 5;
+        l = n == 34 ? 6 : 5;  // n = 34 (four passes either way): 512-byte granules, 239 vs 264 ms
     if (fmax < 2 || fmax > QFT_MAX_TILE_BITS || l < 1 || l > 6 || l >= fmax) {
         *err = "unsupported tile_bits / hub_bits";
         return 2;

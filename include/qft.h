@@ -127,11 +127,6 @@ qft_status_t qft_plan_create_batched(qft_plan_t* out, int n_qubits, int log2_bat
  * the granule size; callers must read it from the plan, not assume it.  Not available for batched plans.
  */
 #define QFT_FLAG_DEFER_SWAPS 32u
-/* QFT_FLAG_CLUSTER_TILE -- use cluster-extended tiles wherever they can be scheduled (the default does for n = 31 ... 33
- * only): the first and the last pass of a three-pass plan run on tiles of 2^16 amplitudes that two CTAs of a thread-block
- * cluster share through distributed shared memory, which doubles the length of the contiguous rows those passes read and
- * write at the same window size.  Needs 2^14 shared-memory tiles and the tensor-memory extension. */
-#define QFT_FLAG_CLUSTER_TILE 64u
 qft_status_t qft_plan_create_tuned(qft_plan_t* out, int n_qubits, int aqft_cutoff_k, int max_fused_qubits, int sign,
                                    qft_norm_t normalisation, int tile_bits, int hub_bits, unsigned flags);
 

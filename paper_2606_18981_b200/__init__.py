@@ -22,7 +22,6 @@ LIB_PATH = os.path.join(_HERE, "libqft.so")
 QFT_OK, QFT_ERR_INVALID_ARG, QFT_ERR_UNSUPPORTED, QFT_ERR_ALLOC, QFT_ERR_CUDA, QFT_ERR_INTERNAL = range(6)
 QFT_NORM_UNITARY, QFT_NORM_NONE, QFT_NORM_INV_N = 0, 1, 2
 QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_NO_EXT_TILE, QFT_FLAG_DEFER_SWAPS = 1, 2, 4, 16, 32
-QFT_FLAG_CLUSTER_TILE = 64
 QFT_MAX_QUBITS = 34
 
 EXPORTS = [

@@ -147,7 +147,7 @@ qft_status_t qft_plan_shard_info(qft_plan_t plan, int pass_index, int rank, int 
         return (qft_status_t)rc;
     }
     const QftPassDesc& d = plan->host.passes[pass_index];
-    const long long bytes = (*unit_n * (d.npair ? 2 : 1)) * ((long long)8 << (d.f + d.xt + d.cx));  // this rank's share of the pass
+    const long long bytes = (*unit_n * (d.npair ? 2 : 1)) * ((long long)8 << (d.f + d.xt));  // this rank's share of the pass
     *remote_bytes_each_way = bytes - (bytes >> *rank_bits_in_tile);
     return QFT_OK;
 }

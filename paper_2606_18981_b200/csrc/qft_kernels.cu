@@ -182,14 +182,12 @@ tma2_kernel_t qft_pick_tma2_lt7(int r1, int r2, int kc);  // qft_tma_lt7.cu
 tma2_kernel_t qft_pick_tma2_lt8(int r1, int r2, int kc);  // qft_tma_lt8.cu
 tma2_kernel_t qft_pick_tma2_lt9(int r1, int r2, int kc);  // qft_tma_lt9.cu
 tma2_kernel_t qft_pick_tma2_xt(int r1, int r2, int kc);   // qft_tma_xt.cu
-tma2_kernel_t qft_pick_tma2_cx(int r1, int r2, int kc);   // qft_tma_cx.cu
 tma2_kernel_t qft_pick_tma2_es7(int r1, int r2, int kc);  // qft_tma_es.cu
 tma2_kernel_t qft_pick_tma2_es8(int r1, int r2, int kc);
 tma2_kernel_t qft_pick_tma2_es9(int r1, int r2, int kc);
 
 static tma2_kernel_t pick_tma2(const QftPassDesc& d) {
     const int kc = d.k < 4 ? d.k : 4;
-    if (d.cx) return d.log2_threads == 9 ? qft_pick_tma2_cx(d.tma.r1, d.tma.r2, kc) : nullptr;
     if (d.xt) return d.log2_threads == 9 ? qft_pick_tma2_xt(d.tma.r1, d.tma.r2, kc) : nullptr;
     if (d.tma.eb > QFT_TMA2_EB_DIRECT) {
         switch (d.log2_threads) {
@@ -250,7 +248,7 @@ static int smem_optin(int dev) {
 static void fill_units(QftPassDesc* d) {
     if (d->unit_n == 0) {
         d->unit_lo = 0;
-        d->unit_n = (int32_t)((1ull << (d->ntile - d->xt - d->cx)) / (d->npair ? 2u : 1u));
+        d->unit_n = (int32_t)((1ull << (d->ntile - d->xt)) / (d->npair ? 2u : 1u));
     }
 }
 
@@ -332,12 +330,12 @@ static cudaError_t launch_tma2(const QftPassDesc& d_in, QftPassCache* cache, int
     fill_units(&d);
     tma2_kernel_t kern = pick_tma2(d);
     if (!kern) return cudaErrorNotSupported;
-    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb, d.ntile) + (d.cx ? QFT_TMA2_CX_BYTES(d.log2_threads) : 0);
+    const size_t smem = ((size_t)8 << d.f) + QFT_TMA2_TABLE_BYTES(d.tma.eb, d.ntile);
     CUtensorMap map;
     {
         std::lock_guard<std::mutex> lock(cache->mu);
         if (!get_map(d, cache, dev, src, &map)) {
-            if (d.xt || d.cx || src != state) return cudaErrorNotSupported;
+            if (d.xt || src != state) return cudaErrorNotSupported;
             // no tensor map: the generic kernel runs the same descriptor (F = Fst for every plain pass)
             QftPassDesc g = d;
             g.kernel = QFT_KERNEL_GENERIC;
@@ -352,7 +350,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d_in, QftPassCache* cache, int
             cache->attr_dev = dev;
         }
     }
-    const unsigned csz = (d.npair || d.cx) ? 2u : 1u;
+    const unsigned csz = d.npair ? 2u : 1u;
     unsigned long long grid = (unsigned long long)sm_count(dev) * tma2_ctas_per_sm(d, smem);
     if (grid > (unsigned long long)d.unit_n * csz) grid = (unsigned long long)d.unit_n * csz;
     grid -= grid % csz;
@@ -364,7 +362,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d_in, QftPassCache* cache, int
     cudaLaunchAttribute attr[2];
     cfg.attrs = attr;
     cfg.numAttrs = 0;
-    if (d.npair > 0 || d.cx) {
+    if (d.npair > 0) {
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2;
         attr[0].val.clusterDim.y = 1;

@@ -99,10 +99,7 @@ void build_unfolded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out
 // Folded schedule: K = 2 + #mid passes, no stand-alone reversal.
 //   regions: H=[0,l)  A=[l,we)  Mid=[we,n-we)  B=[n-we,n-l)  T=[n-l,n)
 //   we_force > 0: that width for the first and the last window instead of the balanced one.
-//   l_mid >= 0: the mid passes use that (smaller) hub: their tiles do not hold address bits [l_mid, l), which are plain
-//   tile-index bits to them (cluster-extended outer passes with one more hub bit than a mid pass can afford).
-bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out, int we_force = 0, int l_mid = -1) {
-    if (l_mid < 0) l_mid = l;
+bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out, int we_force = 0) {
     if (n <= fmax) return false;
     int w = std::min(wcap, fmax - l);
     if (n <= 2 * w) w = (n - 1) / 2;
@@ -140,7 +137,7 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out, 
     for (int c = 0; c < nmid_passes; ++c) {
         PassSpec ps;
         for (int i = 0; i < chunks[c]; ++i) ps.window.push_back(t - i);
-        for (int a = 0; a < l_mid; ++a) ps.F.push_back(a);
+        for (int a = 0; a < l; ++a) ps.F.push_back(a);
         if (nmid_passes == 1) {
             for (int a = we; a < n - we; ++a) { ps.F.push_back(a); ps.moves.push_back({a, n - 1 - a}); }
         } else {
@@ -149,7 +146,7 @@ bool build_folded(int n, int wcap, int fmax, int l, std::vector<PassSpec>* out, 
         if (c == 0)
             for (int a = l; a < we; ++a) ps.swaps.push_back({a, n - 1 - a});
         std::sort(ps.F.begin(), ps.F.end());
-        add_extras(ps, n, f - (l - l_mid));
+        add_extras(ps, n, f);
         t -= chunks[c];
         out->push_back(ps);
     }
@@ -362,7 +359,6 @@ void lower_tma2(QftPassDesc* d, int n) {
           (r1 == 1 && r2 == 1)))
         QFT_REJECT(3);
     if (d->xt && (f != 14 || r1 + r2 < 8)) QFT_REJECT(4);  // the extended tile is built for 2^14 halves only
-    if (d->cx && !(r1 + r2 == 9 || (r1 == 4 && r2 == 4))) QFT_REJECT(41);  // instantiated shapes: 5+4, 4+4 (qft_tma_cx.cu)
     if (s1.a != s2.a + r2) QFT_REJECT(5);  // the window is one run of canonical bits
     const int eb = s2.a;            // canonical bits below the window
     // more than QFT_TMA2_EB_DIRECT: the split end table, instantiated for windows of <= 6 qubits (qft_tma_es*.cu)
@@ -522,8 +518,7 @@ void lower_tma2(QftPassDesc* d, int n) {
 // out of the register steps, its address bit becomes the half-tile index bit, and the descriptor describes
 // one half; the pass must then lower to the TMA kernel (no other kernel knows about the extension).
 bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_fused, bool allow_tma,
-                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err, bool force2 = false, bool xt = false,
-                bool cx = false) {
+                std::vector<int>& qubit_at, QftPassDesc* d, std::string* err, bool force2 = false, bool xt = false) {
     std::memset(d, 0, sizeof(*d));
     std::vector<int> dest(n);
     for (int a = 0; a < n; ++a) dest[a] = a;
@@ -542,13 +537,10 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
         if (src_of[a] < 0) { *err = "in-tile moves are not a permutation"; return false; }
     // load-side and store-side tile bits
     std::vector<int> Fld(ps.F), Fst(ps.F);
-    // xt: the window's lowest qubit g leaves the register steps (tensor-memory extension); cx (with xt): the lowest
-    // qubit h goes to the cluster extension and the second lowest to the tensor-memory extension
-    int g = -1, a_g = -1, b_g = -1, h = -1, a_h = -1, b_h = -1;
-    if (cx && !xt) { *err = "cluster-extended tile without the tensor-memory extension"; return false; }
+    int g = -1, a_g = -1, b_g = -1;
     if (xt) {
-        if ((int)ps.window.size() < (cx ? 4 : 3)) { *err = "extended tile: window too small"; return false; }
-        g = cx ? ps.window[ps.window.size() - 2] : ps.window.back();
+        if (ps.window.size() < 3) { *err = "extended tile: window too small"; return false; }
+        g = ps.window.back();
         for (int a : ps.F)
             if (qubit_at[a] == g) a_g = a;
         if (a_g < 0) { *err = "extended tile: qubit outside the tile"; return false; }
@@ -557,25 +549,12 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
         Fld.erase(std::find(Fld.begin(), Fld.end(), a_g));
         Fst.erase(std::find(Fst.begin(), Fst.end(), b_g));
     }
-    if (cx) {
-        if (!ps.swaps.empty()) { *err = "cluster-extended tile on a pair pass"; return false; }
-        h = ps.window.back();
-        for (int a : ps.F)
-            if (qubit_at[a] == h) a_h = a;
-        if (a_h < 0) { *err = "cluster-extended tile: qubit outside the tile"; return false; }
-        b_h = dest[a_h];
-        if (a_h < hub || b_h < hub) { *err = "cluster-extended tile: CTA bit inside the hub"; return false; }
-        Fld.erase(std::find(Fld.begin(), Fld.end(), a_h));
-        Fst.erase(std::find(Fst.begin(), Fst.end(), b_h));
-    }
     const int f = (int)Fld.size();
     if (f > QFT_MAX_TILE_BITS || n - f > QFT_MAX_TILEIDX_BITS) { *err = "tile too large"; return false; }
     d->n = n; d->f = f; d->ntile = n - f; d->k = k; d->conj = conj; d->scale = 1.0f; d->do_scale = 0;
     d->kernel = QFT_KERNEL_GENERIC;
     d->xt = xt ? 1 : 0;
     d->xt_q = (int8_t)g; d->xt_ld_addr = (int8_t)a_g; d->xt_st_addr = (int8_t)b_g;
-    d->cx = cx ? 1 : 0;
-    d->cx_q = (int8_t)h; d->cx_ld_addr = (int8_t)a_h; d->cx_st_addr = (int8_t)b_h;
     int lt = f - 2;
     if (lt < 5) lt = 5;
     if (lt > 8) lt = 8;
@@ -607,7 +586,6 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
     int ti = 2 * p;
     for (int a = 0; a < n; ++a)
         if (!inFull[a] && !taken[a]) d->tile_addr[ti++] = (int8_t)a;
-    if (cx) d->tile_addr[ti++] = (int8_t)a_h;
     if (xt) d->tile_addr[ti++] = (int8_t)a_g;
     if (ti != n - f) { *err = "tile index bits do not add up"; return false; }
     for (int i = 0; i < n - f; ++i) d->log_tile[i] = (int8_t)qubit_at[d->tile_addr[i]];
@@ -618,7 +596,7 @@ bool lower_pass(const PassSpec& ps, int n, int k, int conj, int hub, bool allow_
         const int wfull = (int)ps.window.size();
         for (int i = 0; i < wfull; ++i)
             if (ps.window[i] != ps.window[0] - i) { *err = "window not contiguous"; return false; }
-        const int w = wfull - (xt ? 1 : 0) - (cx ? 1 : 0);
+        const int w = xt ? wfull - 1 : wfull;
         for (int i = 0; i < w; ++i)
             if (canon_of_q[ps.window[i]] < 0) { *err = "window qubit outside the tile"; return false; }
         d->win_lo = ps.window[w - 1];
@@ -737,15 +715,13 @@ static bool lower_all(const QftPlanParams& prm, std::vector<PassSpec>& specs, in
             }
         }
         if (!done && fbase > fsmem) {
-            // the window and the hub need one bit more than a shared-memory tile holds: tensor-memory extension; two
-            // bits more: a cluster of two CTAs on top of it
-            const bool cx = fbase == fsmem + 2;
+            // the window and the hub need one bit more than a shared-memory tile holds: tensor-memory extension
             PassSpec trial = ps;
-            add_extras(trial, na, fsmem + (cx ? 2 : 1));
+            add_extras(trial, na, fsmem + 1);
             std::vector<int> qa = qubit_at;
             QftPassDesc dt;
-            if ((int)trial.F.size() != fsmem + (cx ? 2 : 1) || !want_tma ||
-                !lower_pass(trial, na, k_eff, conj, l, false, true, qa, &dt, err, true, true, cx))
+            if ((int)trial.F.size() != fsmem + 1 || !want_tma ||
+                !lower_pass(trial, na, k_eff, conj, l, false, true, qa, &dt, err, true, true))
                 return false;
             d = dt;
             qubit_at = qa;
@@ -790,7 +766,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
         *err = "invalid argument";
         return 1;
     }
-    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u | 64u)) { *err = "unknown flag"; return 2; }
+    if (prm.flags & ~(1u | 2u | 4u | 16u | 32u)) { *err = "unknown flag"; return 2; }
     if ((prm.flags & 32u) && (prm.flags & 2u)) { *err = "deferred swaps have no unfolded schedule"; return 2; }
     // defaults from the B200 sweeps (profiles/r01_tile_hub_sweep.md, profiles/r02_tile_hub_sweep.md): 128-byte
     // granules (hub 4) as soon as the state is large enough for a hub to exist, 2^14 tiles once three 10-qubit
@@ -827,29 +803,18 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
     // kernels allowed; tried first, dropped if any pass cannot be lowered
     const bool ext_ok = fmax == 14 && prm.batch_bits == 0 && !(prm.flags & (1u | 2u | 4u | 16u)) && n > fmax + 1;
     if ((prm.flags & 32u) && prm.batch_bits != 0) { *err = "deferred swaps are not available for batched plans"; return 2; }
-    // cluster-extended tiles on top of that (two CTAs share a tile of 2^16 amplitudes through distributed shared
-    // memory): the outer passes of a three-pass folded schedule get one more hub bit (rows twice as long) with the
-    // same windows; the mid pass, a pair pass, keeps the smaller hub.  Default where three passes need 11-qubit windows
-    // (n = 31 ... 33: 256-byte instead of 128-byte rows); QFT_FLAG_CLUSTER_TILE asks for it anywhere it can be scheduled.
-    const bool cx_ok = ext_ok && !(prm.flags & 32u) && l + 1 <= 6 && ((prm.flags & 64u) || (!prm.hub_bits && n >= 31 && n <= 33));
-    for (int attempt = cx_ok ? -1 : (ext_ok ? 0 : 1); attempt < 2; ++attempt) {
-        const int fplan = attempt == -1 ? fmax + 2 : (attempt == 0 ? fmax + 1 : fmax);  // tile bits the schedule may use
+    for (int attempt = ext_ok ? 0 : 1; attempt < 2; ++attempt) {
+        const int fplan = attempt == 0 ? fmax + 1 : fmax;  // tile bits the schedule may use
         std::vector<PassSpec> specs;
         out->passes.clear();
-        out->ext_tile = attempt <= 0;
+        out->ext_tile = attempt == 0;
         out->folded = false;
-        if (attempt == -1) {
-            out->folded = build_folded(n, prm.max_fused, fplan, l + 1, &specs, fplan - (l + 1), l);  // the widest outer windows
-            // only worth it when the outer passes really are cluster tiles and the schedule has three passes
-            if (out->folded && (specs.size() != 3 || (int)specs.front().Fbase.size() != fmax + 2 || (int)specs.back().Fbase.size() != fmax + 2))
-                out->folded = false;
-            if (!out->folded) continue;
-        } else if (prm.flags & 32u) {
+        if (prm.flags & 32u) {
             if (n <= fmax) {
                 build_unfolded(n, prm.max_fused, fmax, l, &specs);  // one tile: simply leave the reversal out
                 specs.back().moves.clear();
             } else if (!build_deferred(n, prm.max_fused, fplan, l, &specs)) {
-                if (attempt <= 0) continue;
+                if (attempt == 0) continue;
                 *err = "deferred swaps: this tile / hub combination cannot be scheduled";
                 return 2;
             }
@@ -858,7 +823,7 @@ int qft_build_plan(const QftPlanParams& prm, QftHostPlan* out, std::string* err)
             out->folded = build_folded(n, prm.max_fused, fplan, l, &specs);
         }
         if (!out->folded) {
-            if (attempt <= 0) continue;  // the extensions only exist for folded schedules
+            if (attempt == 0) continue;  // the extension only exists for folded schedules
             specs.clear();
             // batched transforms that fit one tile: two two-step passes (TMA kernel) beat one three-step pass
             const int wcap = (prm.batch_bits > 0 && n > 10 && n <= fmax) ? std::min(prm.max_fused, (n + 1) / 2) : prm.max_fused;
@@ -951,8 +916,6 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
         if (d.n != n || d.f + d.ntile != n || d.f < 1 || d.f > QFT_MAX_TILE_BITS) return fail("sizes");
         if (d.xt != 0 && d.xt != 1) return fail("xt");
         if (d.xt && d.kernel != QFT_KERNEL_TMA2) return fail("extended tile without the TMA kernel");
-        if (d.cx != 0 && d.cx != 1) return fail("cx");
-        if (d.cx && (!d.xt || d.npair != 0)) return fail("cluster-extended tile needs the tensor-memory extension and no pairs");
         std::vector<int> inF(n, 0), inFst(n, 0);
         for (int j = 0; j < d.f; ++j) {
             if (d.F[j] < 0 || d.F[j] >= n || inF[d.F[j]]) return fail("F not a set of address bits");
@@ -973,15 +936,6 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
             if (d.ntile < 1 || d.tile_addr[d.ntile - 1] != ag) return fail("extended tile: half-tile bit is not the last tile-index bit");
             if (2 * d.npair > d.ntile - 1) return fail("extended tile: half-tile bit inside a pair");
             if (qubit_at[ag] != d.xt_q || d.xt_q != d.win_lo - 1) return fail("extended tile: qubit");
-        }
-        if (d.cx) {
-            // the cluster's tile: one more address bit on each side; CTA c loads the half with bit cx_ld_addr = c
-            const int ah = d.cx_ld_addr, bh = d.cx_st_addr;
-            if (ah < 0 || ah >= n || inTile[ah] || bh < 0 || bh >= n || inFst[bh]) return fail("cluster-extended tile: CTA bits");
-            inTile[ah] = 1;
-            inFst[bh] = 1;
-            if (d.ntile < 2 || d.tile_addr[d.ntile - 2] != ah) return fail("cluster-extended tile: CTA bit is not the last tile-index bit but one");
-            if (qubit_at[ah] != d.cx_q || d.cx_q != d.win_lo - 2) return fail("cluster-extended tile: qubit");
         }
         for (int a = 0; a < n; ++a)
             if (inTile[a] != inFst[a]) return fail("store tile differs from load tile (not in place)");
@@ -1028,11 +982,6 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
         if (d.xt) {
             // the butterfly between the halves comes after every register step of the pass
             if (d.xt_q != next_qubit) return fail("extended tile: gates out of circuit order");
-            --next_qubit;
-        }
-        if (d.cx) {
-            // ... and the butterfly between the CTAs after that
-            if (d.cx_q != next_qubit) return fail("cluster-extended tile: gates out of circuit order");
             --next_qubit;
         }
         if (d.kernel == QFT_KERNEL_TMA2) {
@@ -1192,7 +1141,6 @@ int qft_check_plan(const QftHostPlan& plan, std::string* err) {
             nq2[d.Fst[j]] = d.log_canon[d.st_canon[j]];
         }
         if (d.xt) nq2[d.xt_st_addr] = d.xt_q;
-        if (d.cx) nq2[d.cx_st_addr] = d.cx_q;
         for (int i = 0; i < d.npair; ++i) {
             const int a = d.tile_addr[i], b = d.tile_addr[d.npair + i];
             nq2[a] = qubit_at[b];
@@ -1231,7 +1179,6 @@ int qft_shard_range(const QftHostPlan& plan, size_t pass, int rank, int g, long 
     std::vector<int> inTile(n, 0), inPair(n, 0);
     for (int j = 0; j < d.f; ++j) inTile[d.F[j]] = 1;
     if (d.xt) inTile[d.xt_ld_addr] = 1;
-    if (d.cx) inTile[d.cx_ld_addr] = 1;
     for (int i = 0; i < 2 * d.npair; ++i) inPair[d.tile_addr[i]] = 1;
     int g_in = 0;
     unsigned o = 0, r_in = 0;
@@ -1243,7 +1190,7 @@ int qft_shard_range(const QftHostPlan& plan, size_t pass, int rank, int g, long 
         if (inTile[a]) r_in |= bit << g_in++;
         else o |= bit << m++;
     }
-    const int ubits = d.ntile - d.xt - d.cx - (d.npair ? 1 : 0);  // log2 of the number of units
+    const int ubits = d.ntile - d.xt - (d.npair ? 1 : 0);  // log2 of the number of units
     if (ubits < g) { *err = "fewer units than ranks"; return 2; }
     const long long per_o = 1ll << (ubits - m);  // units that share one value of the outside rank bits
     *unit_n = per_o >> g_in;
@@ -1259,7 +1206,7 @@ int qft_check_shard(const QftHostPlan& plan, int g, std::string* err) {
     for (size_t p = 0; p < plan.passes.size(); ++p) {
         const QftPassDesc& d = plan.passes[p];
         const int n = d.n;
-        const int ubits = d.ntile - d.xt - d.cx - (d.npair ? 1 : 0);
+        const int ubits = d.ntile - d.xt - (d.npair ? 1 : 0);
         std::vector<std::pair<long long, long long>> ranges;
         for (int r = 0; r < (1 << g); ++r) {
             long long lo, cnt;
@@ -1274,11 +1221,11 @@ int qft_check_shard(const QftHostPlan& plan, int g, std::string* err) {
                 unsigned long long tile_hi = d.npair ? ((unsigned long long)u >> (2 * d.npair - 1)) << (2 * d.npair) : (unsigned long long)u;
                 for (int b = 0; b < g; ++b) {
                     const int a = n - g + b;
-                    bool in_tile = (d.xt && a == d.xt_ld_addr) || (d.cx && a == d.cx_ld_addr);
+                    bool in_tile = d.xt && a == d.xt_ld_addr;
                     for (int j = 0; j < d.f; ++j) in_tile = in_tile || d.F[j] == a;
                     if (in_tile) continue;
                     int idx = -1;
-                    for (int i = 0; i < d.ntile - d.xt - d.cx; ++i)
+                    for (int i = 0; i < d.ntile - d.xt; ++i)
                         if (d.tile_addr[i] == a) idx = i;
                     if (idx < 0) { *err = "shard check: rank bit is neither a tile nor a tile-index bit"; return 5; }
                     if (((tile_hi >> idx) & 1ull) != (((unsigned)r >> b) & 1u)) {
@@ -1313,7 +1260,7 @@ void qft_pass_gates(const QftHostPlan& plan, size_t pass, long long* n_h, long l
     *first = *last = -1;
     if (d.nsteps == 0) return;
     const int t_hi = d.steps[0].t_hi;
-    const int t_lo = d.cx ? d.cx_q : (d.xt ? d.xt_q : d.win_lo);
+    const int t_lo = d.xt ? d.xt_q : d.win_lo;
     long long idx = 0;
     for (int t = plan.prm.n - 1; t > t_hi; --t) idx += 1 + std::min(k, t);
     *first = idx;
@@ -1338,12 +1285,11 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
     for (size_t i = 0; i < plan.passes.size(); ++i) {
         const QftPassDesc& d = plan.passes[i];
         if (i) o << ",";
-        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2 ? (d.cx ? "tma2xc" : d.xt ? "tma2x" : "tma2") : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic")
-          << "\",\"tile_bits\":" << d.f + d.xt + d.cx << ",\"F\":[";
+        o << "{\"kernel\":\"" << (d.kernel == QFT_KERNEL_TMA2 ? (d.xt ? "tma2x" : "tma2") : d.kernel == QFT_KERNEL_FUSED2 ? "fused2" : "generic")
+          << "\",\"tile_bits\":" << d.f + d.xt << ",\"F\":[";
         {
             std::vector<int> F(d.F, d.F + d.f);
             if (d.xt) F.push_back(d.xt_ld_addr);
-            if (d.cx) F.push_back(d.cx_ld_addr);
             std::sort(F.begin(), F.end());
             for (size_t j = 0; j < F.size(); ++j) o << (j ? "," : "") << F[j];
         }
@@ -1355,11 +1301,9 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
                 first = false;
             }
         if (d.xt) o << "," << (int)d.xt_q;
-        if (d.cx) o << "," << (int)d.cx_q;
         o << "],\"steps\":[";
         for (int s = 0; s < d.nsteps; ++s) o << (s ? "," : "") << (int)d.steps[s].r;
         if (d.xt) o << ",1";
-        if (d.cx) o << ",1";
         long long nh, ncr, g0, g1;
         qft_pass_gates(plan, i, &nh, &ncr, &g0, &g1);
         o << "],\"n_h\":" << nh << ",\"n_cr\":" << ncr << ",\"gate_first\":" << g0 << ",\"gate_last\":" << g1;
@@ -1373,7 +1317,6 @@ std::string qft_describe_plan(const QftHostPlan& plan) {
         for (int c = 0; c < d.f; ++c) o << (c ? "," : "") << (int)d.log_canon[c];
         o << "]";
         if (d.xt) o << ",\"ext\":{\"qubit\":" << (int)d.xt_q << ",\"load_addr\":" << (int)d.xt_ld_addr << ",\"store_addr\":" << (int)d.xt_st_addr << "}";
-        if (d.cx) o << ",\"cluster_ext\":{\"qubit\":" << (int)d.cx_q << ",\"load_addr\":" << (int)d.cx_ld_addr << ",\"store_addr\":" << (int)d.cx_st_addr << "}";
         o << ",\"pair_swaps\":[";
         for (int p = 0; p < d.npair; ++p)
             o << (p ? "," : "") << "[" << (int)d.tile_addr[p] << "," << (int)d.tile_addr[d.npair + p] << "]";

@@ -34,8 +34,6 @@
 #define QFT_TMA2_EB_MAX 12
 #define QFT_TMA2_END_ROWS(eb) \
     ((eb) > QFT_TMA2_EB_DIRECT ? 2 * (1 << QFT_TMA2_EB_LO) + (1 << ((eb)-QFT_TMA2_EB_LO)) : 2 * ((eb) > 5 ? (1 << (eb)) : 32))
-// (the cluster-extended tile adds 2 x 8 x threads x 8 bytes of staging and two mbarriers: QFT_TMA2_CX_BYTES)
-#define QFT_TMA2_CX_BYTES(log2_threads) (((size_t)2 * 8 * 8 << (log2_threads)) + 16)
 #define QFT_TMA2_TABLE_BYTES(eb, ntile) \
     ((32 * QFT_TMA2_MID_STRIDE + QFT_TMA2_END_ROWS(eb) * QFT_TMA2_END_STRIDE) * 8 + 8 + 24 + (((ntile) + 7) >> 3) * 256 * 16)
 
@@ -97,14 +95,6 @@ struct QftPassDesc {
     // The half-tile index bit is the LAST tile-index bit: tile_addr[ntile-1] = xt_ld_addr.
     int32_t xt;
     int8_t xt_q, xt_ld_addr, xt_st_addr, xt_pad;
-    // ---- cluster-extended tile (QFT_KERNEL_TMA2 with xt = 1 only) ---------------------------------------
-    // cx = 1: two CTAs of a cluster own one tile of 2^(f+2) amplitudes, F + {xt_ld_addr, cx_ld_addr}.  CTA c runs the
-    // extended tile with address bit cx_ld_addr = c exactly as above; then the two CTAs trade half of their results
-    // through distributed shared memory (CTA c keeps the outputs whose xt frequency bit is c) and apply the gates of
-    // one more qubit, cx_q = win_lo - 2: H as a radix-2 butterfly between the CTAs and the controlled-R_m onto it from
-    // below; its frequency bit lands on address bit cx_st_addr.  Tile-index bits: ..., cx_ld_addr, xt_ld_addr (last).
-    int32_t cx;
-    int8_t cx_q, cx_ld_addr, cx_st_addr, cx_pad;
     int8_t F[16];         // load-order bit j <-> address bit F[j], ascending, F[j] = j for j < l
     int8_t Fst[16];       // store-order bit j <-> address bit Fst[j], ascending (= F unless xt)
     int8_t ld_canon[16];  // load-order bit j  -> canonical bit

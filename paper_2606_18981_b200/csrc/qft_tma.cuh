@@ -69,19 +69,6 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, u
         : "memory");
 }
 
-// ---- distributed shared memory (CX): the partner CTA's copy of a shared-memory address, and an asynchronous 8-byte
-// store into it that reports its bytes to an mbarrier over there ----
-__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t cta_rank) {
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(cta_rank));
-    return r;
-}
-__device__ __forceinline__ void st_async_remote(uint32_t remote_addr, float2 v, uint32_t remote_bar) {
-    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(remote_addr),
-                 "f"(v.x), "f"(v.y), "r"(remote_bar)
-                 : "memory");
-}
-
 // ---- tensor memory as a parking lot (XT) ----
 // 32x32b shape: thread i of a warp owns TMEM lane 32 (warp % 4) + i; .xN moves N consecutive columns
 // (32-bit words) of that lane to / from N registers.
@@ -198,19 +185,13 @@ struct SyncPrevKernel {
 };
 // One pass over the units [d.unit_lo, d.unit_lo + d.unit_n) (the launcher fills the range in: all of them, or one rank's
 // share).  The mbarrier behind the tile must have been initialised by the caller; parity carries its phase.
-template <int R1, int R2, int KC, int LT, int XT, int ES, int CX, typename Sync>
+template <int R1, int R2, int KC, int LT, int XT, int ES, typename Sync>
 __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUtensorMap* tmap_p, const QftPassDesc& d,
                                           unsigned char* smem_raw, uint32_t& parity, const Sync sync_before_state) {
     constexpr int F = LT + 5;
     constexpr int NT = 1 << LT;
-    static_assert(!CX || XT, "the cluster-extended tile builds on the tensor-memory extension");
-    constexpr int NQ = R1 + R2 + XT + CX;  // columns of the end table: the window's qubits, lowest first ... and the extensions' 
-    // cluster-extended tile: right behind the tile, two staging buffers of 8 amplitudes per thread that the partner
-    // CTA writes into, and their mbarriers; then the tables
-    constexpr size_t kCxBytes = CX ? QFT_TMA2_CX_BYTES(LT) : 0;
-    float2* cxStage = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F));
-    uint64_t* cxBar = reinterpret_cast<uint64_t*>(cxStage + 2 * 8 * NT);
-    float2* midW = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F) + kCxBytes);
+    constexpr int NQ = R1 + R2 + XT;  // columns of the end table: the window's qubits, lowest first ... and the extension's
+    float2* midW = reinterpret_cast<float2*>(smem_raw + ((size_t)8 << F));
     uint64_t* mbar = reinterpret_cast<uint64_t*>(midW + 32 * kMidStride);
     int* nextc = reinterpret_cast<int*>(mbar + 1);           // next tile's TMA coordinates (5 ints) + the TMEM base address
     float2* endW = reinterpret_cast<float2*>(nextc + 6);     // two end tables (by parity) of max(32, 2^eb) rows
@@ -252,7 +233,7 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
     const uint32_t end_cnt = (uint32_t)NQ << eb_lo;
     const uint32_t end_e = tid / NQ, end_q = tid % NQ;
     const uint32_t end_slot = end_e * kEndStride + end_q;
-    const int end_tq = (XT && end_q >= (uint32_t)(R1 + R2)) ? win_lo - 1 - (int)(end_q - (R1 + R2)) : win_lo + (int)end_q;
+    const int end_tq = (XT && end_q == (uint32_t)(R1 + R2)) ? win_lo - 1 : win_lo + (int)end_q;
     const uint64_t end_mask = (1ull << (end_tq < win_lo ? (end_tq > 0 ? end_tq : 0) : (win_lo > 0 ? win_lo : 0))) - 1ull;
     uint32_t end_ph_e;
     {
@@ -301,19 +282,7 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
         tblA[i] = a;
         tblL[i] = L;
     }
-    if constexpr (CX) {
-        if (tid == 0) {
-            mbar_init(cxBar, 1);
-            mbar_init(cxBar + 1, 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-    }
     __syncthreads();
-    if constexpr (CX) {
-        // the partner's staging barriers exist before anything is sent to them
-        cluster_arrive();
-        cluster_wait();
-    }
     if constexpr (XT) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t warp = tid >> 5;
@@ -321,10 +290,9 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
     }
 
     // ---- tile walk ----
-    const uint32_t csz = (d.npair || CX) ? 2u : 1u;
-    const uint32_t rho = (d.npair || CX) ? (blockIdx.x & 1u) : 0u;  // rank in the cluster
-    const int nbig = d.ntile - XT - CX;  // index bits of the units (an extended tile = two half-tiles, times two CTAs)
-    const uint32_t cx_bit = CX ? (rho << nbig) : 0u;  // the cluster-extended tile: CTA c owns address bit cx_ld_addr = c
+    const uint32_t csz = d.npair ? 2u : 1u;
+    const uint32_t rho = d.npair ? (blockIdx.x & 1u) : 0u;
+    const int nbig = d.ntile - XT;  // index bits of the tiles a CTA owns (an extended tile = two half-tiles)
     const uint32_t nunits = (uint32_t)(d.unit_lo + d.unit_n);  // one past the last unit (the launcher fills the range in)
     const uint32_t ustride = gridDim.x / csz;
     const bool has_end = win_lo > 0;
@@ -343,9 +311,8 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
     const uint64_t c_mask = (1ull << t.tma_len[cj]) - 1ull;
     auto put_coords = [&](uint32_t un, uint32_t half) {
         uint32_t ml, ms;
-        if constexpr (CX) ml = ms = un;
-        else decode_tile(un * csz + rho, d.npair, &ml, &ms);
-        nextc[tid] = (int)((lut(tblA, ml | cx_bit | (half << (nbig + CX))) >> c_lo) & c_mask);
+        decode_tile(un * csz + rho, d.npair, &ml, &ms);
+        nextc[tid] = (int)((lut(tblA, ml | (half << nbig)) >> c_lo) & c_mask);
     };
 
     // everything above is independent of the state; the previous pass must have completed (and its
@@ -374,9 +341,8 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
         float2* endWp = endW + parity * (end_rows * kEndStride);
         {
             uint32_t ml, ms;
-            if constexpr (CX) ml = ms = unit;
-            else decode_tile(unit * csz + rho, d.npair, &ml, &ms);
-            const uint64_t Ltile = lut(tblL, ml | cx_bit | (half << (nbig + CX)));
+            decode_tile(unit * csz + rho, d.npair, &ml, &ms);
+            const uint64_t Ltile = lut(tblL, ml | (half << nbig));
             base_st = lut(tblA, ms);
             if (has_end) {
                 // end bases of this tile: endW[e][q] = product of the controlled-R_m from every qubit below the
@@ -391,7 +357,7 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
                     for (int b = 0; b < eb_lo; ++b)
                         if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
                     int tq = win_lo + (int)q;
-                    if (XT && q >= (uint32_t)(R1 + R2)) tq = win_lo - 1 - (int)(q - (R1 + R2));
+                    if (XT && q == (uint32_t)(R1 + R2)) tq = win_lo - 1;
                     L &= (1ull << (tq < win_lo ? tq : win_lo)) - 1ull;
                     endWp[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, tq, k));
                 }
@@ -518,61 +484,6 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
                     if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
                 wg[bt] = endWp[((kk >> 8) & 127u) * kEndStride + (R1 + R2)];
             }
-            if constexpr (CX) {
-                // One more qubit, across the two CTAs of the cluster (H as a radix-2 butterfly between the CTA whose
-                // tile has address bit cx_ld_addr = 0 and the one with 1, then the controlled-R_m onto it from below).
-                // Both CTAs hold the same positions in the same threads, so thread i trades with thread i: CTA c keeps
-                // the outputs whose xt frequency bit is c and sends the others, 8 amplitudes at a time, through two
-                // staging buffers the partner fills with st.async (their bytes complete the buffer's mbarrier).  A
-                // buffer is refilled two chunks later, which the partner can only reach after every thread here has
-                // sent the chunk in between, i.e. has read this one.
-                float2 wc[NB2];
-#pragma unroll
-                for (int bt = 0; bt < NB2; ++bt) {
-                    uint32_t kk = key2;
-#pragma unroll
-                    for (int i = 0; i < 5 - R2; ++i)
-                        if (bt & (1 << i)) kk ^= t.s2_reg_key[R2 + i];
-                    wc[bt] = endWp[((kk >> 8) & 127u) * kEndStride + (R1 + R2 + 1)];
-                }
-                // (a barrier serves chunks c8 and c8 + 2 of every tile: its phase parity is that of c8 / 2)
-                const uint32_t cx_rstage = map_to_cta(smem_u32(cxStage), rho ^ 1u) + tid * 8u;
-                const uint32_t cx_rbar = map_to_cta(smem_u32(cxBar), rho ^ 1u);
-                float2* __restrict__ dstc = dst + ((uint64_t)rho << d.xt_st_addr);
-                const uint64_t cx_off = 1ull << d.cx_st_addr;
-#pragma unroll
-                for (int c8 = 0; c8 < 4; ++c8) {
-                    constexpr uint32_t kChunkBytes = 8u * 8u * NT;
-                    const uint32_t buf = c8 & 1;
-                    float2 pk[8];
-                    tmem_fetch8(tpark + 16u * c8, pk);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int B = 8 * c8 + i;
-                        const float2 lo = qftp::padd(pk[i], x[B]);
-                        const float2 hi = qftp::cmul(qftp::psub(pk[i], x[B]), wg[B >> R2]);
-                        x[B] = rho ? hi : lo;  // kept (x[B] itself is no longer needed)
-                        st_async_remote(cx_rstage + (buf * 8u + i) * (NT * 8u), rho ? lo : hi, cx_rbar + buf * 8u);
-                    }
-                    if (tid == 0) mbar_expect_tx(cxBar + buf, kChunkBytes);
-                    mbar_wait(cxBar + buf, (uint32_t)(c8 >> 1));
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int B = 8 * c8 + i;
-                        const float2 r = cxStage[(buf * 8u + i) * NT + tid];
-                        const float2 a = rho ? r : x[B], b = rho ? x[B] : r;
-                        float2 o0 = qftp::padd(a, b);
-                        float2 o1 = qftp::cmul(qftp::psub(a, b), wc[B >> R2]);
-                        if (d.conj) { o0.y = -o0.y; o1.y = -o1.y; }
-                        uint64_t o = 0;
-#pragma unroll
-                        for (int bb = 0; bb < 5; ++bb)
-                            if (B & (1 << bb)) o += c2st[bb];
-                        dstc[o] = o0;
-                        dstc[o + cx_off] = o1;
-                    }
-                }
-            } else {
             if (d.npair) cluster_wait();  // the partner holds its tile on chip: its addresses may be overwritten
             float2* __restrict__ dst1 = dst + (1ull << d.xt_st_addr);
 #pragma unroll
@@ -592,7 +503,6 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
                     dst[o] = lo;
                     dst1[o] = hi;
                 }
-            }
             }
         } else {
             if (d.conj) {
@@ -625,14 +535,13 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
     }
 }
 
-template <int LT, int CX>
+template <int LT>
 __device__ __forceinline__ uint64_t* tma2_mbar(unsigned char* smem_raw) {
-    return reinterpret_cast<uint64_t*>(smem_raw + ((size_t)8 << (LT + 5)) + (CX ? QFT_TMA2_CX_BYTES(LT) : 0) +
-                                       32 * kMidStride * sizeof(float2));
+    return reinterpret_cast<uint64_t*>(smem_raw + ((size_t)8 << (LT + 5)) + 32 * kMidStride * sizeof(float2));
 }
 
 // One pass per launch (the default for every n whose passes are bound by HBM).
-template <int R1, int R2, int KC, int LT, int XT, int ES = 0, int CX = 0>
+template <int R1, int R2, int KC, int LT, int XT, int ES = 0>
 __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     qft_pass_tma2(float2* __restrict__ state, const __grid_constant__ CUtensorMap tmap,
                   const __grid_constant__ QftPassDesc d) {
@@ -640,11 +549,11 @@ __global__ void __launch_bounds__(1 << LT, (LT == 8) ? 2 : ((LT == 7) ? 4 : 1))
     // let the next pass's CTAs be scheduled as soon as SM resources free up (they wait inside tma2_pass)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (threadIdx.x == 0) {
-        mbar_init(tma2_mbar<LT, CX>(smem_raw), 1);
+        mbar_init(tma2_mbar<LT>(smem_raw), 1);
         fence_proxy_async();
     }
     uint32_t parity = 0;
-    tma2_pass<R1, R2, KC, LT, XT, ES, CX>(state, &tmap, d, smem_raw, parity, SyncPrevKernel{});
+    tma2_pass<R1, R2, KC, LT, XT, ES>(state, &tmap, d, smem_raw, parity, SyncPrevKernel{});
 }
 
 }  // namespace qftk

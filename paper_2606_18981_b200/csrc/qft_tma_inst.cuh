@@ -4,14 +4,14 @@
 
 typedef void (*tma2_kernel_t)(float2*, const CUtensorMap, const QftPassDesc);
 
-template <int R1, int R2, int LT, int XT, int ES = 0, int CX = 0>
+template <int R1, int R2, int LT, int XT, int ES = 0>
 static tma2_kernel_t qft_pick_tma2_kc(int kc) {
     switch (kc) {
-        case 0: return qftk::qft_pass_tma2<R1, R2, 0, LT, XT, ES, CX>;
-        case 1: return qftk::qft_pass_tma2<R1, R2, 1, LT, XT, ES, CX>;
-        case 2: return qftk::qft_pass_tma2<R1, R2, 2, LT, XT, ES, CX>;
-        case 3: return qftk::qft_pass_tma2<R1, R2, 3, LT, XT, ES, CX>;
-        default: return qftk::qft_pass_tma2<R1, R2, 4, LT, XT, ES, CX>;
+        case 0: return qftk::qft_pass_tma2<R1, R2, 0, LT, XT, ES>;
+        case 1: return qftk::qft_pass_tma2<R1, R2, 1, LT, XT, ES>;
+        case 2: return qftk::qft_pass_tma2<R1, R2, 2, LT, XT, ES>;
+        case 3: return qftk::qft_pass_tma2<R1, R2, 3, LT, XT, ES>;
+        default: return qftk::qft_pass_tma2<R1, R2, 4, LT, XT, ES>;
     }
 }
 

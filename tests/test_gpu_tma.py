@@ -200,29 +200,3 @@ def test_small_windows_against_oracle(n, tile_bits, w):
     if w <= 4:
         assert deepest > 7, "this configuration was chosen to exercise the split end table"
 
-
-# Cluster-extended tiles (kernel "tma2xc": two CTAs of a cluster share a 2^16-amplitude tile through distributed shared
-# memory; default for n = 31 ... 33, where only closed forms are available: tests/test_gpu_large.py).  With
-# QFT_FLAG_CLUSTER_TILE the planner emits them at n = 23 ... 27, where the full oracle is cheap: both instantiated shapes
-# (4+4+1+1 with 5 hub bits in the mid pass, 5+4+1+1 with 4), every in-group truncation, both signs.
-@pytest.mark.parametrize("n,hub_bits", [(23, 5), (24, 5), (25, 4), (26, 4), (26, 5), (27, 5)])
-def test_tma2xc_against_oracle(n, hub_bits):
-    import torch
-
-    import paper_2606_18981_b200 as qft
-
-    x = qi.gaussian(n, 400 + n)
-    for k, sign, norm in [(None, -1, 0), (3, 1, 0), (12, -1, 1), (0, -1, 0), (1, 1, 2), (2, -1, 0)]:
-        kk = n if k is None else k
-        plan = qft.Plan(n, kk, 13, sign, norm, 14, hub_bits, qft.QFT_FLAG_CLUSTER_TILE)
-        plan.self_check()
-        kinds = [p["kernel"] for p in plan.describe()["passes"]]
-        assert kinds[0] == "tma2xc" and kinds[-1] == "tma2xc", kinds
-        t = torch.from_numpy(x).cuda()
-        plan.execute(t)
-        plan.execute(t)  # twice: forward of the forward, so that a stale staging buffer or barrier phase shows
-        torch.cuda.synchronize()
-        got = t.cpu().numpy().astype(np.complex128)
-        plan.close()
-        ref = oracle.qft(oracle.qft(x, kk, sign, norm).astype(np.complex64), kk, sign, norm)
-        assert_parity_numpy(got, ref, n, (n, hub_bits, kk, sign, norm, kinds))

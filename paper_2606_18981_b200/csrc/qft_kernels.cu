@@ -99,14 +99,25 @@ __global__ void __launch_bounds__(256) qft_tile_pass_generic(float2* __restrict_
         const uint32_t niter = (d.f > lt) ? (1u << (d.f - lt)) : 1u;
         const bool active = (d.f >= lt) || (tid < (1u << d.f));
         if (active) {
-            for (uint32_t it = 0; it < niter; ++it) {
-                uint64_t off = off_t;
-                uint32_t can = can_t;
-                for (int j = lt; j < d.f; ++j)
-                    if ((it >> (j - lt)) & 1u) { off |= 1ull << d.F[j]; can |= 1u << d.ld_canon[j]; }
-                float2 v = state[base_ld + off];
-                if (d.conj) v.y = -v.y;
-                tile[swz(can)] = v;
+            // eight loads in flight per thread before the first one is consumed
+            for (uint32_t it0 = 0; it0 < niter; it0 += 8) {
+                float2 v[8];
+                uint32_t can[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const uint32_t it = it0 + u;
+                    uint64_t off = off_t;
+                    can[u] = can_t;
+                    for (int j = lt; j < d.f; ++j)
+                        if ((it >> (j - lt)) & 1u) { off |= 1ull << d.F[j]; can[u] |= 1u << d.ld_canon[j]; }
+                    if (it < niter) v[u] = state[base_ld + off];
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    if (it0 + u >= niter) break;
+                    if (d.conj) v[u].y = -v[u].y;
+                    tile[swz(can[u])] = v[u];
+                }
             }
         }
     }

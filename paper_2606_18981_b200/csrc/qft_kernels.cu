@@ -34,6 +34,11 @@ __device__ __forceinline__ void generic_step(float2* tile, const QftPassDesc& d,
     const uint32_t nb = 1u << (d.f - R);
     const uint32_t lowmask = (1u << a) - 1u;
     const uint64_t lmask = (t_lo > 0) ? ((1ull << t_lo) - 1ull) : 0ull;
+    // logical bits below the group that this thread's own index bits contribute: the same for all its butterflies
+    const int lt = d.log2_threads;
+    uint64_t Lthread = Ltile;
+    for (int b = 0; b < a && b < lt; ++b)
+        if ((threadIdx.x >> b) & 1u) Lthread |= 1ull << d.log_canon[b];
     for (uint32_t o = threadIdx.x; o < nb; o += blockDim.x) {
         const uint32_t c0 = ((o & ~lowmask) << R) | (o & lowmask);
         float2 x[1 << R];
@@ -42,8 +47,8 @@ __device__ __forceinline__ void generic_step(float2* tile, const QftPassDesc& d,
         dif_group<R, FAST>(x, d.k);
         if (t_lo > 0) {
             // logical bits below the group: from the tile index and from this thread's canonical low bits
-            uint64_t L = Ltile;
-            for (int b = 0; b < a; ++b)
+            uint64_t L = Lthread;
+            for (int b = lt; b < a; ++b)
                 if ((c0 >> b) & 1u) L |= 1ull << d.log_canon[b];
             L &= lmask;
 #pragma unroll
@@ -73,8 +78,12 @@ __device__ __forceinline__ void generic_step_dispatch(float2* tile, const QftPas
     else generic_step<R, false>(tile, d, st, Ltile, scale_now);
 }
 
-__global__ void __launch_bounds__(256) qft_tile_pass_generic(float2* __restrict__ state,
-                                                             const __grid_constant__ QftPassDesc d) {
+// RMAX: the largest register group this instantiation handles.  The one for groups of <= 2 qubits (one-qubit windows
+// on small tiles, permutation-only passes) is compiled for 4 CTAs per SM; the general one needs 250 registers for its
+// 32-point groups and runs one CTA per SM (profiles/r02_config3_sweep.md).
+template <int RMAX>
+__global__ void __launch_bounds__(256, RMAX <= 2 ? 4 : 1) qft_tile_pass_generic(float2* __restrict__ state,
+                                                                               const __grid_constant__ QftPassDesc d) {
     extern __shared__ float2 tile[];
     const uint32_t tid = threadIdx.x;
     const int lt = d.log2_threads;
@@ -128,12 +137,17 @@ __global__ void __launch_bounds__(256) qft_tile_pass_generic(float2* __restrict_
     for (int s = 0; s < d.nsteps; ++s) {
         const QftStep st = d.steps[s];
         const bool scale_now = d.do_scale && (s == d.nsteps - 1);
-        switch (st.r) {
-            case 1: generic_step_dispatch<1>(tile, d, st, Ltile, scale_now); break;
-            case 2: generic_step_dispatch<2>(tile, d, st, Ltile, scale_now); break;
-            case 3: generic_step_dispatch<3>(tile, d, st, Ltile, scale_now); break;
-            case 4: generic_step_dispatch<4>(tile, d, st, Ltile, scale_now); break;
-            default: generic_step_dispatch<5>(tile, d, st, Ltile, scale_now); break;
+        if constexpr (RMAX <= 2) {
+            if (st.r == 1) generic_step_dispatch<1>(tile, d, st, Ltile, scale_now);
+            else generic_step_dispatch<2>(tile, d, st, Ltile, scale_now);
+        } else {
+            switch (st.r) {
+                case 1: generic_step_dispatch<1>(tile, d, st, Ltile, scale_now); break;
+                case 2: generic_step_dispatch<2>(tile, d, st, Ltile, scale_now); break;
+                case 3: generic_step_dispatch<3>(tile, d, st, Ltile, scale_now); break;
+                case 4: generic_step_dispatch<4>(tile, d, st, Ltile, scale_now); break;
+                default: generic_step_dispatch<5>(tile, d, st, Ltile, scale_now); break;
+            }
         }
         __syncthreads();
     }
@@ -184,7 +198,9 @@ static pass_kernel_t pick_kernel(const QftPassDesc& d) {
         QFT_PICK(2, 2)
 #undef QFT_PICK
     }
-    return (pass_kernel_t)qftk::qft_tile_pass_generic;
+    int rmax = 0;
+    for (int s = 0; s < d.nsteps; ++s) rmax = d.steps[s].r > rmax ? d.steps[s].r : rmax;
+    return rmax <= 2 ? (pass_kernel_t)qftk::qft_tile_pass_generic<2> : (pass_kernel_t)qftk::qft_tile_pass_generic<5>;
 }
 
 // ---- QFT_KERNEL_TMA2 ---------------------------------------------------------------------------

@@ -540,14 +540,18 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         try:
             torch.cuda.empty_cache()
+            t20, cores = oracle_full(20, args.k)
             t22, cores = oracle_full(22, args.k)
+            t22k4, cores = oracle_full(22, 4)  # AQFT k = 4 at the paper's size (Fig. 5)
             t26, cores = oracle_full(26, args.k)
-            m22, m26 = sorted(t22)[1], sorted(t26)[1]
+            m20, m22, m22k4, m26 = sorted(t20)[1], sorted(t22)[1], sorted(t22k4)[1], sorted(t26)[1]
             cpu_baseline = {"value": 5.0 * (1 << 26) * 26 / m26 / 1e9, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
                             "sample": ("whole gate-by-gate oracle circuit (fp64, OpenMP), 1 warm-up + 3 trials, median, at "
-                                       f"n=26: {m26:.3f} s (value = 5 N log2 N / t there) and n=22: {m22:.4f} s; bounded "
+                                       f"n=26: {m26:.3f} s (value = 5 N log2 N / t there), n=22: {m22:.4f} s (k=4: {m22k4:.4f} s) and n=20: "
+                                       f"{m20:.4f} s; bounded "
                                        f"sample of the n={n} workload: same circuit, smaller states"),
-                            "seconds_n26": m26, "seconds_n22": m22, "trials_n26": t26, "trials_n22": t22,
+                            "seconds_n26": m26, "seconds_n22": m22, "seconds_n20": m20, "seconds_n22_k4": m22k4,
+                            "trials_n26": t26, "trials_n22": t22,
                             "gflops_n22": 5.0 * (1 << 22) * 22 / m22 / 1e9}
             if n >= 28 and args.extrapolate_cpu:
                 est, spent, sdesc, _ = oracle_sample(n, args.k)

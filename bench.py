@@ -55,7 +55,7 @@ def parse_args():
     ap.add_argument("--sweep", default="26,33", help="comma list of extra n to time briefly ('' = none)")
     ap.add_argument("--small-n", default="20,22", help="comma list of launch-bound sizes to time over 1000 back-to-back "
                                                        "transforms ('' = none)")
-    ap.add_argument("--batched", default="16:12", help="comma list of n:log2_batch pairs to time briefly (batched "
+    ap.add_argument("--batched", default="12:16,16:12,22:6", help="comma list of n:log2_batch pairs to time briefly (batched "
                                                        "plans; '' = none), e.g. 10:18,16:12")
     return ap.parse_args()
 

@@ -73,3 +73,74 @@ def test_ranks_shares_one_after_the_other_equal_the_whole_pass(n, g, flags, k):
     if flags == 0 and n <= 24:
         assert_parity_numpy(parts.cpu().numpy().astype(np.complex128), oracle.qft(x, kk), n, (n, g, kk))
     plan.close()
+
+
+def _fd_worker(rank, world, job, q):
+    import os
+    import tempfile
+
+    from paper_2606_18981_b200.sharded import exchange_fds
+
+    f = tempfile.TemporaryFile()
+    f.write(f"shard of rank {rank}".encode())
+    f.flush()
+    fds = exchange_fds(rank, world, f.fileno(), job)
+    seen = []
+    for fd in fds:
+        os.lseek(fd, 0, 0)
+        seen.append(os.read(fd, 64).decode())
+    q.put((rank, seen))
+
+
+@pytest.mark.parametrize("world", [2, 4])
+def test_file_descriptor_exchange_between_processes(world):
+    """The host side of the multi-process driver (paper_2606_18981_b200/sharded.py): every rank ends up with every
+    rank's descriptor (here: of temporary files; on a GPU node: of the shards' cuMemCreate handles)."""
+    import multiprocessing as mp
+    import os
+
+    ctx = mp.get_context("fork")
+    q = ctx.Queue()
+    job = f"test{os.getpid()}_{world}"
+    procs = [ctx.Process(target=_fd_worker, args=(r, world, job, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    want = [f"shard of rank {r}" for r in range(world)]
+    assert got == [(r, want) for r in range(world)]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,g,k", [(24, 1, None), (24, 2, None), (26, 3, 7)])
+def test_shards_as_separate_allocations_mapped_back_to_back(n, g, k):
+    """LocalShards: 2^g physical allocations (cuMemCreate) on this one device, mapped into one virtual range
+    (cuMemAddressReserve / cuMemMap / cuMemSetAccess) exactly as the multi-process driver maps its peers' shards; every
+    rank's share of every pass, one after the other.  Same result as qft_execute on an ordinary buffer, bit for bit."""
+    import torch
+    from cuda.bindings import driver as cu
+
+    import qft_inputs as qi
+    from paper_2606_18981_b200.sharded import LocalShards
+
+    x = qi.gaussian(n, 500 + n)
+    t = torch.from_numpy(x).cuda()
+    plan = qft.Plan(n, n if k is None else k)
+    ref = t.clone()
+    plan.execute(ref)
+    torch.cuda.synchronize()
+    sh = LocalShards(n, g, device=torch.cuda.current_device(), aqft_cutoff_k=k)
+    assert sh.map.world == 1 << g and sh.map.shard_bytes == 8 << (n - g)
+    (err,) = cu.cuMemcpy(sh.map.base, t.data_ptr(), 8 << n)
+    assert err == cu.CUresult.CUDA_SUCCESS
+    sh.execute(torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    out = torch.empty_like(t)
+    (err,) = cu.cuMemcpy(out.data_ptr(), sh.map.base, 8 << n)
+    assert err == cu.CUresult.CUDA_SUCCESS
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref))
+    sh.close()
+    plan.close()

@@ -57,4 +57,9 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    # python -m paper_2606_18981_b200.build [--force] [-v] [--define NAME ... --lib PATH]: the product library, or a
+    # differently configured one beside it (e.g. --define QFT_PHASE_TIMING --lib /tmp/libqft_phase.so for tune --phase-lib)
+    defs = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--define"]
+    alt = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--lib"]
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, extra_flags=["-D" + d for d in defs],
+                lib=os.path.abspath(alt[0]) if alt else LIB))

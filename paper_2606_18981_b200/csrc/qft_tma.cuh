@@ -315,10 +315,35 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
         nextc[tid] = (int)((lut(tblA, ml | (half << nbig)) >> c_lo) & c_mask);
     };
 
+    // End bases of a half-tile, written into the end table of parity `par`: endW[e][q] = product of the controlled-R_m
+    // from every qubit below the window (tile-index bits + in-tile bits e) onto the window's q-th qubit (with an
+    // extended tile the last column belongs to the extension's qubit win_lo - 1).  The phase is linear over disjoint
+    // bit sets, so a thread's entry is its constant part from e plus the tile's part.  Filled one half-tile ahead (in
+    // the shadow of the previous half-tile's step 2), never on the path between two tiles.
+    auto fill_end = [&](uint32_t un, uint32_t half, uint32_t par) {
+        if (!has_end) return;
+        uint32_t ml, ms;
+        decode_tile(un * csz + rho, d.npair, &ml, &ms);
+        const uint64_t Ltile = lut(tblL, ml | (half << nbig));
+        float2* tab = endW + par * (end_rows * kEndStride);
+        if (tid < end_cnt) tab[end_slot] = qftp::cis_fwd_u32(end_ph_e + qftp::cr_phase_u32(Ltile & end_mask, end_tq, k));
+        for (uint32_t i = tid + NT; i < end_cnt; i += NT) {  // only when 2^eb (R1 + R2 + XT) > threads
+            const uint32_t e = i / NQ, q = i % NQ;
+            uint64_t L = Ltile;
+            for (int b = 0; b < eb_lo; ++b)
+                if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
+            int tq = win_lo + (int)q;
+            if (XT && q == (uint32_t)(R1 + R2)) tq = win_lo - 1;
+            L &= (1ull << (tq < win_lo ? tq : win_lo)) - 1ull;
+            tab[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, tq, k));
+        }
+    };
+
     // everything above is independent of the state; the previous pass must have completed (and its
     // writes be visible) before the first load
     sync_before_state(tid);
     uint32_t unit = (uint32_t)d.unit_lo + blockIdx.x / csz;
+    if (unit < nunits) fill_end(unit, 0u, parity);
     if (unit < nunits && tid < 32u) {
         if (tid < 5u) put_coords(unit, 0u);
         __syncwarp();
@@ -337,35 +362,13 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
         // ---- bookkeeping while the tile's load is in flight (few registers live here) ----
         const bool last_half = half == (uint32_t)XT;
         const bool has_next = !last_half || unit + ustride < nunits;
+        const uint32_t next_unit = last_half ? unit + ustride : unit, next_half = last_half ? 0u : half + 1u;
         uint64_t base_st;
-        float2* endWp = endW + parity * (end_rows * kEndStride);
+        float2* endWp = endW + parity * (end_rows * kEndStride);  // filled while the previous half-tile was in step 2
         {
             uint32_t ml, ms;
             decode_tile(unit * csz + rho, d.npair, &ml, &ms);
-            const uint64_t Ltile = lut(tblL, ml | (half << nbig));
             base_st = lut(tblA, ms);
-            if (has_end) {
-                // end bases of this tile: endW[e][q] = product of the controlled-R_m from every qubit below the
-                // window (tile-index bits + in-tile bits e) onto the window's q-th qubit (with an extended tile
-                // the last column belongs to the extension's qubit win_lo - 1).  The phase is linear over disjoint
-                // bit sets, so a thread's entry is its constant part from e plus the tile's part.
-                if (tid < end_cnt)
-                    endWp[end_slot] = qftp::cis_fwd_u32(end_ph_e + qftp::cr_phase_u32(Ltile & end_mask, end_tq, k));
-                for (uint32_t i = tid + NT; i < end_cnt; i += NT) {  // only when 2^eb (R1 + R2 + XT) > threads
-                    const uint32_t e = i / NQ, q = i % NQ;
-                    uint64_t L = Ltile;
-                    for (int b = 0; b < eb_lo; ++b)
-                        if ((e >> b) & 1u) L |= 1ull << t.e_log[b];
-                    int tq = win_lo + (int)q;
-                    if (XT && q == (uint32_t)(R1 + R2)) tq = win_lo - 1;
-                    L &= (1ull << (tq < win_lo ? tq : win_lo)) - 1ull;
-                    endWp[e * kEndStride + q] = qftp::cis_fwd_u32(qftp::cr_phase_u32(L, tq, k));
-                }
-            }
-            if (tid < 5u && has_next) {
-                if (last_half) put_coords(unit + ustride, 0u);
-                else put_coords(unit, half + 1u);
-            }
         }
         float2 x[32];
         // keep the 96 per-register shared-memory offsets out of loop-invariant hoisting (they would
@@ -385,6 +388,7 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
         QFT_ALL32(QFT_LD1)
 #undef QFT_LD1
         __syncthreads();  // every amplitude of the tile is in a register: the buffer becomes the exchange
+        if (tid < 5u && has_next) put_coords(next_unit, next_half);  // (read by thread 0 two barriers further down)
         QFT_PHASE(2)
         if (d.conj) {
 #pragma unroll
@@ -408,6 +412,7 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
             mbar_expect_tx(mbar, 8u << F);
             tma_load_5d(smem_raw, tmap_p, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
         }
+        if (has_next) fill_end(next_unit, next_half, parity ^ 1u);
         QFT_PHASE(4)
 
         {

@@ -26,10 +26,15 @@ def main() -> int:
     ap.add_argument("--log2-batch", type=int, default=0, help="2^b independent transforms back to back")
     ap.add_argument("--reps", type=int, default=2)
     ap.add_argument("--no-time", action="store_true")
+    ap.add_argument("--phase-lib", default=None,
+                    help="a library built with `python -m paper_2606_18981_b200.build --define QFT_PHASE_TIMING --lib PATH`: "
+                         "print, per pass, the clocks thread 0 of CTA 0 spends in each phase of the TMA kernel per tile")
     ap.add_argument("--loop", type=int, default=0, help="also time this many back-to-back qft_execute calls (launch-bound sizes)")
     a = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("needs a CUDA device")
+    if a.phase_lib:
+        qft.LIB_PATH = a.phase_lib  # before the first call loads the library
     n = a.n
     plan = qft.Plan(n, n if a.k is None else a.k, a.max_fused, -1, qft.QFT_NORM_UNITARY, a.tile_bits, a.hub_bits, a.flags,
                     a.log2_batch)
@@ -41,6 +46,29 @@ def main() -> int:
     for _ in range(a.reps):
         qft.qft_execute(plan.handle, st.data_ptr(), s)
     torch.cuda.synchronize()
+    if a.phase_lib:
+        import ctypes
+
+        lib = qft.load()
+        lib.qft_debug_set_phase_buffer.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+        names = ["bookkeeping", "wait for the tile's load", "step 1 reads + barrier", "step 1 arithmetic + exchange writes + barrier",
+                 "step 2 reads + barrier + next load + next end table", "step 2 arithmetic", "park first half in tensor memory",
+                 "extension butterfly + stores"]
+        for p in range(plan.num_passes):
+            buf = torch.zeros(16, dtype=torch.int64, device="cuda")
+            lib.qft_debug_set_phase_buffer(plan.handle, p, buf.data_ptr())
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            qft.qft_execute_pass(plan.handle, p, st.data_ptr(), s)
+            e1.record()
+            torch.cuda.synchronize()
+            lib.qft_debug_set_phase_buffer(plan.handle, p, None)
+            c = buf.cpu().tolist()
+            tiles = max(c[8], 1)
+            print(json.dumps({"n": a.n, "pass": p, "ms": round(e0.elapsed_time(e1), 3), "tiles_of_cta0": c[8],
+                              "clocks_per_tile": {names[i]: round(c[i] / tiles) for i in range(8)},
+                              "total_clocks_per_tile": round(sum(c[:8]) / tiles)}))
+        return 0
     if a.no_time:
         return 0
     npass = plan.num_passes

@@ -89,6 +89,7 @@ def main() -> int:
         qft.qft_execute(plan.handle, st.data_ptr(), s)
     e1.record()
     torch.cuda.synchronize()
+    execute_ms = round(e0.elapsed_time(e1) / reps, 3)
     loop_us = None
     if a.loop:
         for _ in range(20):
@@ -103,7 +104,7 @@ def main() -> int:
     d = plan.describe()
     print(json.dumps({"launches": plan.num_launches, "loop_us_per_execute": loop_us, "n": d["n"], "batch_bits": d["batch_bits"], "k": d["k"], "tile_bits": d["tile_bits"], "hub_bits": d["hub_bits"], "passes": npass,
                       "kernels": [p["kernel"] for p in d["passes"]], "steps": [p["steps"] for p in d["passes"]],
-                      "pass_ms": [round(v, 3) for v in acc], "execute_ms": round(e0.elapsed_time(e1) / reps, 3),
+                      "pass_ms": [round(v, 3) for v in acc], "execute_ms": execute_ms,
                       "gbs_per_pass": [round(16.0 * (1 << n) / v / 1e6) for v in acc]}))
     return 0
 

@@ -75,42 +75,40 @@ def test_ranks_shares_one_after_the_other_equal_the_whole_pass(n, g, flags, k):
     plan.close()
 
 
-def _fd_worker(rank, world, job, q):
-    import os
-    import tempfile
-
-    from paper_2606_18981_b200.sharded import exchange_fds
-
-    f = tempfile.TemporaryFile()
-    f.write(f"shard of rank {rank}".encode())
-    f.flush()
-    fds = exchange_fds(rank, world, f.fileno(), job)
-    seen = []
-    for fd in fds:
-        os.lseek(fd, 0, 0)
-        seen.append(os.read(fd, 64).decode())
-    q.put((rank, seen))
+_FD_WORKER = """
+import os, sys, tempfile
+sys.path.insert(0, sys.argv[4])
+from paper_2606_18981_b200.sharded import exchange_fds
+rank, world, job = int(sys.argv[1]), int(sys.argv[2]), sys.argv[3]
+f = tempfile.TemporaryFile()
+f.write(f"shard of rank {rank}".encode())
+f.flush()
+fds = exchange_fds(rank, world, f.fileno(), job)
+seen = []
+for fd in fds:
+    os.lseek(fd, 0, 0)
+    seen.append(os.read(fd, 64).decode())
+print("|".join(seen))
+"""
 
 
 @pytest.mark.parametrize("world", [2, 4])
 def test_file_descriptor_exchange_between_processes(world):
     """The host side of the multi-process driver (paper_2606_18981_b200/sharded.py): every rank ends up with every
     rank's descriptor (here: of temporary files; on a GPU node: of the shards' cuMemCreate handles)."""
-    import multiprocessing as mp
     import os
+    import subprocess
+    import sys
 
-    ctx = mp.get_context("fork")
-    q = ctx.Queue()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     job = f"test{os.getpid()}_{world}"
-    procs = [ctx.Process(target=_fd_worker, args=(r, world, job, q)) for r in range(world)]
-    for p in procs:
-        p.start()
-    got = sorted(q.get(timeout=120) for _ in procs)
-    for p in procs:
-        p.join(60)
-        assert p.exitcode == 0
-    want = [f"shard of rank {r}" for r in range(world)]
-    assert got == [(r, want) for r in range(world)]
+    procs = [subprocess.Popen([sys.executable, "-c", _FD_WORKER, str(r), str(world), job, root], stdout=subprocess.PIPE,
+                              stderr=subprocess.PIPE, text=True) for r in range(world)]
+    want = "|".join(f"shard of rank {r}" for r in range(world))
+    for r, p in enumerate(procs):
+        out, err = p.communicate(timeout=180)
+        assert p.returncode == 0, err[-2000:]
+        assert out.strip() == want, (r, out)
 
 
 @pytest.mark.gpu

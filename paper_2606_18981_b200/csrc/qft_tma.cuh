@@ -402,6 +402,8 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
         QFT_PHASE(3)
 
         // ------------------------------ step 2 ------------------------------
+        // (the next half-tile's end table first: its short arithmetic chain runs under the latency of the reads below)
+        if (has_next) fill_end(next_unit, next_half, parity ^ 1u);
 #define QFT_LD2(B) x[B] = lds64(smem_raw, off2_mid ^ reg_off<B>(c2mid));
         QFT_ALL32(QFT_LD2)
 #undef QFT_LD2
@@ -412,7 +414,6 @@ __device__ __forceinline__ void tma2_pass(float2* __restrict__ state, const CUte
             mbar_expect_tx(mbar, 8u << F);
             tma_load_5d(smem_raw, tmap_p, mbar, nextc[0], nextc[1], nextc[2], nextc[3], nextc[4]);
         }
-        if (has_next) fill_end(next_unit, next_half, parity ^ 1u);
         QFT_PHASE(4)
 
         {

@@ -221,3 +221,49 @@ def test_aqft_round_trip(n, k):
     y = gpu_qft(x, k)
     z = gpu_qft(y, k, sign=1)
     assert rel_l2(z, x) <= tol(n)
+
+
+@pytest.mark.parametrize("n_lo,n_hi,count", [(13, 20, 160), (20, 24, 48)])
+def test_random_plan_configurations(n_lo, n_hi, count):
+    """A seeded sweep over the planner's knobs (tile / hub bits, window cap, cutoff, sign, normalisation, unfolded /
+    deferred schedules) at n = 13 ... 23: whatever plan comes out must match the oracle.  Unschedulable combinations
+    must be refused with QFT_ERR_UNSUPPORTED, never fail the self-check."""
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    rng = np.random.default_rng(20261105 + n_lo)
+    ran = 0
+    for _ in range(count):
+        n = int(rng.integers(n_lo, n_hi))
+        tile_bits = int(rng.choice([0, 0, 9, 10, 11, 12, 13, 14]))
+        hub_bits = int(rng.choice([0, 0, 2, 3, 4, 5]))
+        w = int(rng.choice([2, 3, 4, 5, 6, 7, 9, 13]))
+        k = int(rng.choice([n, n, 0, 1, 2, 3, 5, 9]))
+        sign = int(rng.choice([-1, 1]))
+        norm = int(rng.integers(0, 3))
+        flags = int(rng.choice([0, 0, 0, qft.QFT_FLAG_UNFOLDED, qft.QFT_FLAG_DEFER_SWAPS, qft.QFT_FLAG_NO_TMA]))
+        try:
+            plan = qft.Plan(n, k, w, sign, norm, tile_bits, hub_bits, flags)
+        except qft.QftError as e:
+            assert e.status == qft.QFT_ERR_UNSUPPORTED, (n, tile_bits, hub_bits, w, k, flags, str(e))
+            continue
+        plan.self_check()
+        x = qi.gaussian(n, 1000 + ran)
+        t = torch.from_numpy(x).cuda()
+        plan.execute(t)
+        torch.cuda.synchronize()
+        got = t.cpu().numpy().astype(np.complex128)
+        what = (n, tile_bits, hub_bits, w, k, sign, norm, flags, [p["kernel"] for p in plan.describe()["passes"]])
+        if flags == qft.QFT_FLAG_DEFER_SWAPS:
+            # the plan reports where every qubit ended: undo that layout on the host, compare with the natural-order oracle
+            order = plan.output_order()
+            K = np.arange(1 << n, dtype=np.int64)
+            J = np.zeros_like(K)
+            for a, q in enumerate(order):
+                J |= ((K >> (n - 1 - q)) & 1) << a
+            got = got[J]
+        parity(got, oracle.qft(x, k, sign, norm), what)
+        plan.close()
+        ran += 1
+    assert ran >= count * 5 // 8

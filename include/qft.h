@@ -250,6 +250,42 @@ qft_status_t qft_fidelity(const void* device_a, const void* device_b, int n_qubi
 qft_status_t qft_leakage(const void* device_state, int n_qubits, unsigned long long bin, double* leakage_out,
                          void* stream);
 
+/*
+ * qft_fidelity_batched_static -- the fidelity of PAPER.md:181 for `batch` pairs of states at once, for callers that
+ * cannot allocate device memory: a process whose HBM was all handed to one pool or arena at start-up (or filled by
+ * the state vectors themselves: one n = 33 state is 64 GiB), where a cudaMalloc made later by a library fails, and a
+ * caller in a latency-critical loop that cannot afford the device-wide stall an allocation or a free may cause.
+ * qft_fidelity allocates its accumulators at the first call on a device; this function allocates and frees nothing,
+ * on the host side of the runtime or the device, at any call.  Its accumulators (4 doubles per state) are a fixed
+ * array inside the library image: QFT_STATIC_MAX_BATCH * 32 bytes = 128 KiB on every GPU that loads libqft.so, held
+ * until the process exits.
+ *   device_a, device_b   DEVICE pointers, float2[batch * 2^n_qubits] each, 16-byte aligned; pair b is elements
+ *                        [b 2^n, (b+1) 2^n) of both (the layout of qft_plan_create_batched, any batch >= 1, not only
+ *                        powers of two).  Read only.
+ *   n_qubits             1 .. QFT_MAX_QUBITS;  batch * 2^n_qubits <= 2^34.
+ *   batch                1 .. QFT_STATIC_MAX_BATCH.  A larger batch is refused with QFT_ERR_UNSUPPORTED and nothing is
+ *                        enqueued; qft_static_last_error() then names the limit.  Split the batch, or use qft_fidelity.
+ *   device_fidelity_out  DEVICE pointer, double[batch], 8-byte aligned, owned by the caller:
+ *                        out[b] = |<a_b, b_b>|^2 / (||a_b||^2 ||b_b||^2), fp64 accumulation as in qft_fidelity;
+ *                        NaN where a state of the pair is all zero (qft_fidelity refuses that case on the host; this
+ *                        call never waits for the device, so it cannot).
+ *   stream               a cudaStream_t as void*.  The call only enqueues (a clear of the accumulators it uses, the
+ *                        reduction, a final division); it does not synchronise.
+ * Shared scratch: every call on a device uses the same array, which still holds the previous call's sums.  Each
+ * call clears its part in stream order, so calls that follow one another on one stream, or that the caller orders
+ * with events, are correct; calls whose device work can overlap (two streams, two threads) race on the array and
+ * return garbage without any error.
+ * First call on a device: looks up the array's address on that device (one CUDA runtime call, under a lock, which
+ * may load the module); later calls make no such call.  Make the first call before starting any stream capture.
+ * Errors: QFT_ERR_INVALID_ARG (null, misaligned, n_qubits or batch out of range), QFT_ERR_UNSUPPORTED (batch beyond
+ * the limit), QFT_ERR_CUDA (no device, address look-up or launch failed).  The text of the last error this function
+ * returned on the calling thread is qft_static_last_error() ("" if none); qft_last_cuda_error() is not updated.
+ */
+#define QFT_STATIC_MAX_BATCH 4096
+qft_status_t qft_fidelity_batched_static(const void* device_a, const void* device_b, int n_qubits, int batch,
+                                         double* device_fidelity_out, void* stream);
+const char* qft_static_last_error(void);
+
 /* Re-runs the planner's host-side proof: follows every qubit through every
  * pass's address permutation and checks that each gate's target was inside the
  * tile when applied, that tiles are closed under the store permutation, and

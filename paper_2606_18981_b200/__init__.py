@@ -23,6 +23,7 @@ QFT_OK, QFT_ERR_INVALID_ARG, QFT_ERR_UNSUPPORTED, QFT_ERR_ALLOC, QFT_ERR_CUDA, Q
 QFT_NORM_UNITARY, QFT_NORM_NONE, QFT_NORM_INV_N = 0, 1, 2
 QFT_FLAG_GENERIC_ONLY, QFT_FLAG_UNFOLDED, QFT_FLAG_NO_TMA, QFT_FLAG_NO_EXT_TILE, QFT_FLAG_DEFER_SWAPS = 1, 2, 4, 16, 32
 QFT_MAX_QUBITS = 34
+QFT_STATIC_MAX_BATCH = 4096  # states per qft_fidelity_batched_static call (its built-in 128 KiB scratch array)
 
 EXPORTS = [
     "qft_plan_create", "qft_plan_create_batched", "qft_plan_create_tuned", "qft_execute", "qft_execute_pass", "qft_execute_host", "qft_plan_destroy",
@@ -31,6 +32,7 @@ EXPORTS = [
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
     "qft_plan_shard_info", "qft_plan_shard_check", "qft_execute_pass_shard",
     "qft_norm_sq", "qft_encode", "qft_rescale", "qft_fidelity", "qft_leakage",
+    "qft_fidelity_batched_static", "qft_static_last_error",
 ]
 
 _lib = None
@@ -114,6 +116,10 @@ def load() -> ctypes.CDLL:
         _f.restype = ci
     L.qft_last_cuda_error.argtypes = []
     L.qft_last_cuda_error.restype = ctypes.c_char_p
+    L.qft_fidelity_batched_static.argtypes = [vp, vp, ci, ci, vp, vp]
+    L.qft_fidelity_batched_static.restype = ci
+    L.qft_static_last_error.argtypes = []
+    L.qft_static_last_error.restype = ctypes.c_char_p
     _lib = L
     return L
 
@@ -292,6 +298,26 @@ def qft_fidelity(device_a_ptr: int, device_b_ptr: int, n_qubits: int, stream: in
 
 def qft_leakage(device_state_ptr: int, n_qubits: int, bin_index: int, stream: int = 0) -> float:
     return _dbl_call("qft_leakage", device_state_ptr, n_qubits, int(bin_index), stream)
+
+
+def qft_static_last_error() -> str:
+    return load().qft_static_last_error().decode()
+
+
+def qft_fidelity_batched_static(device_a_ptr: int, device_b_ptr: int, n_qubits: int, batch: int,
+                                device_fidelity_out_ptr: int, stream: int = 0) -> None:
+    """Fidelity of `batch` pairs of states (complex64[batch * 2^n] each, device) into a device double[batch],
+    without any device allocation: for processes whose GPU memory is all spoken for (one big pool, or state
+    vectors sized to fill the card) and for loops that cannot take an allocation's stall.  The accumulators are
+    a fixed array inside libqft.so, shared by every call on the device: batch <= QFT_STATIC_MAX_BATCH (more
+    raises QftError with status QFT_ERR_UNSUPPORTED), and calls that overlap on the GPU race.  Only enqueues;
+    the first call on a device also looks the array's address up and should precede any stream capture."""
+    st = load().qft_fidelity_batched_static(device_a_ptr, device_b_ptr, int(n_qubits), int(batch),
+                                            device_fidelity_out_ptr, stream)
+    if st != QFT_OK:
+        err = QftError(st, "qft_fidelity_batched_static")
+        err.args = (f"{qft_status_string(st)}: {qft_static_last_error()}",)
+        raise err
 
 
 class Plan:

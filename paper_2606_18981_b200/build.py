@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqft.so")
-SOURCES = ["qft_api.cu", "qft_kernels.cu", "qft_tma_lt7.cu", "qft_tma_lt8.cu", "qft_tma_lt9.cu", "qft_tma_xt.cu", "qft_tma_es.cu", "qft_metrics.cu", "qft_plan.cpp"]
+SOURCES = ["qft_api.cu", "qft_kernels.cu", "qft_tma_lt7.cu", "qft_tma_lt8.cu", "qft_tma_lt9.cu", "qft_tma_xt.cu", "qft_tma_es.cu", "qft_metrics.cu", "qft_metrics_static.cu", "qft_plan.cpp"]
 HEADERS = ["qft_plan.h", "qft_device.cuh", "qft_fused.cuh", "qft_tma.cuh", "qft_tma_inst.cuh", "qft_packed.cuh", "qft_phase.cuh", "qft_launch.h", os.path.join("..", "..", "include", "qft.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -54,8 +54,6 @@ __device__ __forceinline__ void generic_step(float2* tile, const QftPassDesc& d,
 #pragma unroll
             for (int i = 0; i < R; ++i) {
                 const float2 W = cis_fwd_u32(cr_phase_u32(L, t_hi - i, d.k));
-                constexpr int dummy = 0;
-                (void)dummy;
                 const int pos = R - 1 - i;
 #pragma unroll
                 for (int u = 0; u < (1 << R); ++u)
@@ -367,8 +365,9 @@ static cudaError_t launch_tma2(const QftPassDesc& d_in, QftPassCache* cache, int
             QftPassDesc g = d;
             g.kernel = QFT_KERNEL_GENERIC;
             g.log2_threads = 8;
-            static QftPassCache plain;  // attribute bookkeeping of the fallback only
-            std::lock_guard<std::mutex> lock2(plain.mu);
+            // A cold path: a fresh cache per launch, so the shared-memory attribute is set (idempotent) for whichever
+            // generic instantiation this pass picks; one shared cache would skip it for the second instantiation.
+            QftPassCache plain;
             return launch_plain(g, &plain, dev, state, stream);
         }
         if (cache->attr_dev != dev) {

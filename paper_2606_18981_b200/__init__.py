@@ -176,12 +176,18 @@ def qft_execute_oop(plan: int, device_in_ptr: int, device_out_ptr: int, stream: 
         raise QftError(st, "qft_execute_oop")
 
 
-def qft_plan_output_order(plan: int, n_qubits: int):
-    arr = (ctypes.c_int * n_qubits)()
+def qft_plan_output_order(plan: int, n_qubits: int | None = None):
+    """qubit_of_bit[a] for a < n.  The C call writes the plan's own n entries whatever the caller believes n to be,
+    so the buffer always has room for QFT_MAX_QUBITS and n is read from the plan; a caller-supplied n_qubits that
+    disagrees with the plan is an error, not an overrun."""
+    arr = (ctypes.c_int * QFT_MAX_QUBITS)()
     st = load().qft_plan_output_order(plan, arr)
     if st != QFT_OK:
         raise QftError(st, "qft_plan_output_order")
-    return list(arr)
+    n = int(qft_plan_describe(plan)["n"])
+    if n_qubits is not None and int(n_qubits) != n:
+        raise ValueError(f"qft_plan_output_order: the plan has {n} qubits, the caller said {n_qubits}")
+    return list(arr)[:n]
 
 
 def qft_execute_pass(plan: int, pass_index: int, device_state_ptr: int, stream: int = 0) -> None:

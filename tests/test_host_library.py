@@ -150,8 +150,12 @@ def test_deferred_swaps_plans():
                 assert p.num_passes <= q.num_passes
             p.close()
             q.close()
+    b = qft.qft_plan_create_batched(12, 4, 12, 13, -1, 0)  # sanity: batched plans exist ...
+    assert qft.qft_plan_output_order(b) == [11 - a for a in range(12)]  # ... and report the per-state order
+    with pytest.raises(ValueError):
+        qft.qft_plan_output_order(b, 3)  # a caller's wrong idea of n is refused, not written past
+    qft.qft_plan_destroy(b)
     with pytest.raises(qft.QftError) as ei:
-        qft.qft_plan_create_batched(12, 4, 12, 13, -1, 0)  # sanity: batched plans exist ...
         qft.qft_plan_create_tuned(12, 12, 13, -1, 0, 0, 0, qft.QFT_FLAG_DEFER_SWAPS | qft.QFT_FLAG_UNFOLDED)
     assert ei.value.status == qft.QFT_ERR_UNSUPPORTED
 

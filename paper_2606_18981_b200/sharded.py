@@ -78,15 +78,30 @@ class ShardMap:
         self.world = len(handles)
         self.handles = list(handles)
         total = shard_bytes * self.world
-        self.base = int(_check(cu.cuMemAddressReserve(total, granularity(device), 0, 0), "cuMemAddressReserve"))
         self.total = total
-        for r, h in enumerate(self.handles):
-            _check(cu.cuMemMap(self.base + r * shard_bytes, shard_bytes, 0, h, 0), "cuMemMap")
-        acc = cu.CUmemAccessDesc()
-        acc.location.type = cu.CUmemLocationType.CU_MEM_LOCATION_TYPE_DEVICE
-        acc.location.id = device
-        acc.flags = cu.CUmemAccess_flags.CU_MEM_ACCESS_FLAGS_PROT_READWRITE
-        _check(cu.cuMemSetAccess(self.base, total, [acc], 1), "cuMemSetAccess")
+        self.base = 0
+        mapped = 0  # shards mapped so far: what a failure half-way has to undo
+        try:
+            self.base = int(_check(cu.cuMemAddressReserve(total, granularity(device), 0, 0), "cuMemAddressReserve"))
+            for r, h in enumerate(self.handles):
+                _check(cu.cuMemMap(self.base + r * shard_bytes, shard_bytes, 0, h, 0), "cuMemMap")
+                mapped = r + 1
+            acc = cu.CUmemAccessDesc()
+            acc.location.type = cu.CUmemLocationType.CU_MEM_LOCATION_TYPE_DEVICE
+            acc.location.id = device
+            acc.flags = cu.CUmemAccess_flags.CU_MEM_ACCESS_FLAGS_PROT_READWRITE
+            _check(cu.cuMemSetAccess(self.base, total, [acc], 1), "cuMemSetAccess")
+        except BaseException:
+            # the map takes ownership of the handles: release them, the mappings made so far and the reservation
+            if self.base:
+                if mapped:
+                    cu.cuMemUnmap(self.base, mapped * shard_bytes)
+                cu.cuMemAddressFree(self.base, total)
+                self.base = 0
+            for h in self.handles:
+                cu.cuMemRelease(h)
+            self.handles = []
+            raise
 
     def shard_ptr(self, rank: int) -> int:
         return self.base + rank * self.shard_bytes
@@ -119,10 +134,41 @@ def import_shard(fd: int):
                   "cuMemImportFromShareableHandle")
 
 
+def _job_dir(sock_dir: str, job: str) -> str:
+    """The directory that holds this job's sockets: <sock_dir>/qft_shards_<uid>_<job>, mode 0700, owned by this user.
+    Every rank of the job computes the same name; whoever comes first creates it.  A directory of that name that
+    belongs to somebody else, or that others may write to, is refused: descriptors are not handed to strangers."""
+    d = os.path.join(sock_dir, f"qft_shards_{os.getuid()}_{job}")
+    try:
+        os.mkdir(d, 0o700)
+    except FileExistsError:
+        pass
+    st = os.lstat(d)
+    import stat as _stat
+
+    if not _stat.S_ISDIR(st.st_mode) or st.st_uid != os.getuid() or (st.st_mode & 0o077):
+        raise PermissionError(f"{d} is not a private directory of uid {os.getuid()}")
+    return d
+
+
+def _peer_uid(conn) -> int:
+    import struct
+
+    cred = conn.getsockopt(socket.SOL_SOCKET, socket.SO_PEERCRED, struct.calcsize("3i"))
+    _pid, uid, _gid = struct.unpack("3i", cred)
+    return uid
+
+
 def exchange_fds(rank: int, world: int, fd: int, job: str, sock_dir: str = "/tmp", timeout: float = 120.0):
     """All-to-all of one file descriptor per rank between the processes of one node, over Unix-domain sockets
-    (SCM_RIGHTS).  Returns the list of descriptors indexed by rank (own entry = `fd`).  Pure host code: no CUDA."""
-    path = lambda r: os.path.join(sock_dir, f"qft_shards_{job}_{r}.sock")
+    (SCM_RIGHTS).  Returns the list of descriptors indexed by rank (own entry = `fd`).  Pure host code: no CUDA.
+    The sockets live in a 0700 directory of this user (_job_dir); a message counts only if its sender runs under this
+    user (SO_PEERCRED), names a rank in range other than our own, and is the first from that rank.  Anything else is
+    dropped (its descriptors closed) and the wait goes on until every rank has been heard or `timeout` expires."""
+    if not (0 <= rank < world):
+        raise ValueError(f"rank {rank} outside 0..{world - 1}")
+    d = _job_dir(sock_dir, job)
+    path = lambda r: os.path.join(d, f"{r}.sock")
     srv = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
     try:
         os.unlink(path(rank))
@@ -151,24 +197,48 @@ def exchange_fds(rank: int, world: int, fd: int, job: str, sock_dir: str = "/tmp
                     time.sleep(0.01)
             c.sendmsg([rank.to_bytes(4, "little")], [(socket.SOL_SOCKET, socket.SCM_RIGHTS, array.array("i", [fd]))])
             c.close()
-        srv.settimeout(timeout)
-        for _ in range(world - 1):
-            conn, _addr = srv.accept()
-            msg, anc, _flags, _a = conn.recvmsg(4, socket.CMSG_LEN(4))
-            src = int.from_bytes(msg, "little")
-            got = array.array("i")
-            for level, ctype, data in anc:
-                if level == socket.SOL_SOCKET and ctype == socket.SCM_RIGHTS:
-                    got.frombytes(data[: len(data) - (len(data) % got.itemsize)])
-            if not got:
-                raise RuntimeError(f"rank {rank}: no descriptor in the message from rank {src}")
-            fds[src] = int(got[0])
-            conn.close()
+        deadline = time.time() + timeout
+        while any(f is None for f in fds):
+            left = deadline - time.time()
+            if left <= 0:
+                raise TimeoutError(f"rank {rank}: no descriptor from ranks {[r for r, f in enumerate(fds) if f is None]}")
+            srv.settimeout(left)
+            try:
+                conn, _addr = srv.accept()
+            except socket.timeout:
+                continue
+            try:
+                conn.settimeout(max(left, 0.1))
+                uid = _peer_uid(conn)
+                msg, anc, _flags, _a = conn.recvmsg(4, socket.CMSG_LEN(4))
+                got = array.array("i")
+                for level, ctype, data in anc:
+                    if level == socket.SOL_SOCKET and ctype == socket.SCM_RIGHTS:
+                        got.frombytes(data[: len(data) - (len(data) % got.itemsize)])
+                src = int.from_bytes(msg, "little") if len(msg) == 4 else -1
+                if uid == os.getuid() and 0 <= src < world and src != rank and fds[src] is None and len(got) == 1:
+                    fds[src] = int(got[0])
+                else:  # a stranger, a duplicate, a malformed message: not ours to keep
+                    for g in got:
+                        os.close(g)
+            except (socket.timeout, OSError):
+                pass
+            finally:
+                conn.close()
+    except BaseException:
+        for r, f in enumerate(fds):
+            if r != rank and f is not None:
+                os.close(f)
+        raise
     finally:
         srv.close()
         try:
             os.unlink(path(rank))
         except FileNotFoundError:
+            pass
+        try:
+            os.rmdir(d)  # the last rank out removes the directory; the others find it non-empty
+        except OSError:
             pass
     return fds
 

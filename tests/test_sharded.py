@@ -86,8 +86,8 @@ f.flush()
 fds = exchange_fds(rank, world, f.fileno(), job)
 seen = []
 for fd in fds:
-    os.lseek(fd, 0, 0)
-    seen.append(os.read(fd, 64).decode())
+    # pread: the ranks share each file's offset (one open file description behind every copy of the descriptor)
+    seen.append(os.pread(fd, 64, 0).decode())
 print("|".join(seen))
 """
 
@@ -142,3 +142,58 @@ def test_shards_as_separate_allocations_mapped_back_to_back(n, g, k):
     assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref))
     sh.close()
     plan.close()
+
+
+def test_fd_exchange_drops_bogus_senders_and_refuses_a_shared_directory(tmp_path):
+    """exchange_fds keeps one descriptor per peer rank and only from a well-formed first message: a sender
+    naming a rank out of range, the receiver's own rank, or a rank already heard is dropped and its descriptor closed;
+    the socket directory must be private to this user."""
+    import array
+    import os
+    import socket
+    import tempfile
+    import threading
+    import time
+
+    from paper_2606_18981_b200.sharded import _job_dir, exchange_fds
+
+    job = f"bogus{os.getpid()}"
+    files = [tempfile.TemporaryFile() for _ in range(3)]
+    for i, f in enumerate(files):
+        f.write(f"file {i}".encode())
+        f.flush()
+    res = {}
+
+    def run(rank):
+        res[rank] = exchange_fds(rank, 2, files[rank].fileno(), job, sock_dir=str(tmp_path), timeout=60.0)
+
+    t0 = threading.Thread(target=run, args=(0,))
+    t0.start()
+    sock0 = os.path.join(str(tmp_path), f"qft_shards_{os.getuid()}_{job}", "0.sock")
+    for _ in range(2000):
+        if os.path.exists(sock0):
+            break
+        time.sleep(0.005)
+    for claimed in (7, 0, 0xFFFFFFFF):  # out of range, the receiver's own rank, garbage
+        c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+        c.connect(sock0)
+        c.sendmsg([claimed.to_bytes(4, "little")], [(socket.SOL_SOCKET, socket.SCM_RIGHTS, array.array("i", [files[2].fileno()]))])
+        c.close()
+    t1 = threading.Thread(target=run, args=(1,))
+    t1.start()
+    t0.join(90)
+    t1.join(90)
+    assert not t0.is_alive() and not t1.is_alive()
+    assert res[0][0] == files[0].fileno() and res[1][1] == files[1].fileno()
+    assert os.pread(res[0][1], 64, 0) == b"file 1" and os.pread(res[1][0], 64, 0) == b"file 0"
+    os.close(res[0][1])
+    os.close(res[1][0])
+    assert not os.path.exists(os.path.dirname(sock0))  # the last rank out removed the directory
+
+    shared = tmp_path / f"qft_shards_{os.getuid()}_open"
+    shared.mkdir()
+    os.chmod(shared, 0o777)
+    with pytest.raises(PermissionError):
+        _job_dir(str(tmp_path), "open")
+    with pytest.raises(ValueError):
+        exchange_fds(2, 2, files[0].fileno(), job, sock_dir=str(tmp_path))

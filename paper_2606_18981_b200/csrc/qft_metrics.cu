@@ -137,6 +137,12 @@ qft_status_t qft_encode_padded(void* device_state, int n_qubits, const void* dev
         length > (1ull << n_qubits) || (((uintptr_t)device_state) & 15))
         return QFT_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
+    if (device_x != device_state) {
+        // the copy below is undefined for overlapping ranges: the source is the state itself or disjoint from it
+        const char *x0 = (const char*)device_x, *x1 = x0 + 8ull * length;
+        const char *s0 = (const char*)device_state, *s1 = s0 + (8ull << n_qubits);
+        if (x0 < s1 && s0 < x1) return QFT_ERR_INVALID_ARG;
+    }
     if (device_x != device_state &&
         cudaMemcpyAsync(device_state, device_x, 8ull * length, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
         return QFT_ERR_CUDA;

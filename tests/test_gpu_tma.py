@@ -127,9 +127,10 @@ def test_plan_reuse_across_streams_and_states():
     torch.cuda.synchronize()
     ref = oracle.qft(xa)
     got = ta.cpu().numpy().astype(np.complex128)
-    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 1e-4
+    # seven transforms in a row on ta, six on tb: rounding adds in quadrature (about sqrt(7) x 3e-7), inside the bounds
+    assert_parity_numpy(got, ref, n, "reuse across streams: forward after three round trips")
     back = tb.cpu().numpy().astype(np.complex128)
-    assert float(np.linalg.norm(back - xb) / np.linalg.norm(xb)) <= 1e-4
+    assert_parity_numpy(back, xb.astype(np.complex128), n, "reuse across streams: three round trips")
     fwd.close()
     inv.close()
 
@@ -156,7 +157,7 @@ def test_execute_is_cuda_graph_capturable():
     torch.cuda.synchronize()
     ref = oracle.qft(x)
     got = t.cpu().numpy().astype(np.complex128)
-    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 2e-5
+    assert_parity_numpy(got, ref, n, "graph replay")
     # replay on fresh data gives the transform of the fresh data
     y = qi.gaussian(n, 5)
     t.copy_(torch.from_numpy(y).cuda())
@@ -164,7 +165,7 @@ def test_execute_is_cuda_graph_capturable():
     torch.cuda.synchronize()
     ref = oracle.qft(y)
     got = t.cpu().numpy().astype(np.complex128)
-    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 2e-5
+    assert_parity_numpy(got, ref, n, "graph replay on fresh data")
     plan.close()
 
 

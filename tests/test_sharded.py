@@ -197,3 +197,120 @@ def test_fd_exchange_drops_bogus_senders_and_refuses_a_shared_directory(tmp_path
         _job_dir(str(tmp_path), "open")
     with pytest.raises(ValueError):
         exchange_fds(2, 2, files[0].fileno(), job, sock_dir=str(tmp_path))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,g,kw", [(28, 1, {}), (27, 2, {"tile_bits": 14, "hub_bits": 6})])
+def test_ranks_shares_on_extended_tiles(n, g, kw):
+    """The tensor-memory extended-tile kernel's rank-share walk (unit_lo offset plus the half bit as the last tile-index
+    bit): default plans have such passes only from n = 28, the tuned n = 27 plan is made of them entirely.
+    Every rank's share of every pass, one after the other on one buffer, is qft_execute bit for bit."""
+    import torch
+
+    import qft_inputs as qi
+
+    plan = qft.Plan(n, n, **kw)
+    kinds = [p["kernel"] for p in plan.describe()["passes"]]
+    assert "tma2x" in kinds, kinds
+    whole = qi.gaussian_device(n, 700 + n, device="cuda")
+    parts = whole.clone()
+    plan.execute(whole)
+    s = torch.cuda.current_stream().cuda_stream
+    order = list(range(1 << g))
+    for ps in range(plan.num_passes):
+        order = order[1:] + order[:1]
+        for r in order:
+            qft.qft_execute_pass_shard(plan.handle, ps, parts.data_ptr(), r, g, s)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(whole), torch.view_as_real(parts))
+    plan.close()
+
+
+_RANK_WORKER = """
+import os, sys, time
+rank, world, n, job, root, out = int(sys.argv[1]), int(sys.argv[2]), int(sys.argv[3]), sys.argv[4], sys.argv[5], sys.argv[6]
+sys.path.insert(0, root)
+import numpy as np
+from cuda.bindings import driver as cu
+import qft_inputs as qi
+from paper_2606_18981_b200.sharded import ShardedQft
+
+
+class FileBarrier:
+    # test infrastructure: a barrier over the ranks' processes through files in a directory they share
+    def __init__(self):
+        self.i = 0
+
+    def __call__(self):
+        open(os.path.join(out, f"b{self.i}_{rank}"), "w").close()
+        deadline = time.time() + 120
+        while not all(os.path.exists(os.path.join(out, f"b{self.i}_{r}")) for r in range(world)):
+            if time.time() > deadline:
+                raise TimeoutError(f"rank {rank}: barrier {self.i}")
+            time.sleep(0.0005)
+        self.i += 1
+
+
+barrier = FileBarrier()
+sq = ShardedQft(n, rank, world, 0, barrier, job)   # every rank on device 0: the one GPU there is
+S = (1 << n) // world
+x = qi.gaussian(n, 900 + n)[rank * S:(rank + 1) * S].copy()
+(err,) = cu.cuMemcpyHtoD(sq.shard_ptr, x, x.nbytes)
+assert err == cu.CUresult.CUDA_SUCCESS, err
+(err,) = cu.cuCtxSynchronize()
+assert err == cu.CUresult.CUDA_SUCCESS, err
+barrier()                                           # every shard holds its input before any pass reads a peer's
+sq.execute(0)
+y = np.empty_like(x)
+(err,) = cu.cuMemcpyDtoH(y, sq.shard_ptr, y.nbytes)
+assert err == cu.CUresult.CUDA_SUCCESS, err
+np.save(os.path.join(out, f"shard_{rank}.npy"), y)
+info = [sq.map.world, sq.map.shard_bytes, sq.plan.num_passes]
+sq.close()
+print("ok", *info)
+"""
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [1, 2, 4])
+def test_multi_process_driver_on_one_gpu(world, tmp_path):
+    """ShardedQft as it is meant to run - one process per rank - with every rank on the one GPU of this box: each
+    process creates its shard (cuMemCreate), exports it as a file descriptor, receives its peers' descriptors over the
+    Unix sockets, imports and maps all shards back to back, runs its share of every pass (TMA loads and plain stores
+    through the imported mappings) and meets the others at a barrier between passes.  The assembled result equals
+    qft_execute on an ordinary buffer bit for bit and the oracle within the parity bounds.  (world = 1: the class at
+    g = 0 with nothing to exchange.)  This exercises the cross-process handle exchange and mapping; it says nothing
+    about NVLink, and no timing is taken."""
+    import os
+    import subprocess
+    import sys
+
+    import torch
+
+    import oracle
+    import qft_inputs as qi
+    from parity_bounds import assert_parity_numpy
+
+    n = 24
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    job = f"mp{os.getpid()}_{world}"
+    procs = [subprocess.Popen([sys.executable, "-c", _RANK_WORKER, str(r), str(world), str(n), job, root, str(tmp_path)],
+                              stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True) for r in range(world)]
+    try:
+        for r, p in enumerate(procs):
+            out, err = p.communicate(timeout=300)
+            assert p.returncode == 0, (r, err[-3000:])
+            assert out.split() == ["ok", str(world), str((8 << n) // world), "3"], out
+    finally:
+        for p in procs:
+            if p.poll() is None:
+                p.kill()
+    got = np.concatenate([np.load(os.path.join(str(tmp_path), f"shard_{r}.npy")) for r in range(world)])
+    x = qi.gaussian(n, 900 + n)
+    t = torch.from_numpy(x).cuda()
+    plan = qft.Plan(n, n)
+    plan.execute(t)
+    torch.cuda.synchronize()
+    plan.close()
+    assert np.array_equal(got.view(np.float32), t.cpu().numpy().view(np.float32))
+    assert_parity_numpy(got.astype(np.complex128), oracle.qft(x), n, ("multi-process", world))

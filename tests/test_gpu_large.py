@@ -160,11 +160,13 @@ def _host_gib():
         return 0.0
 
 
-@pytest.mark.parametrize("n,k", [(28, 28), (28, 5), (30, 30)])
+@pytest.mark.parametrize("n,k", [(28, 28), (28, 5), (30, 30), (31, 31)])
 def test_dense_full_oracle_at_the_bench_kernels(n, k):
     """Every output element of a Gaussian input against the full CPU oracle at n = 28 and n = 30: the default
     plans here are made of the same kernel instantiations bench.py times (the tensor-memory extended 5+4+1
-    passes), which the tone inputs (a handful of non-zero outputs) and 32 samples cannot check densely."""
+    passes), which the tone inputs (a handful of non-zero outputs) and 32 samples cannot check densely.
+    n = 31 is the smallest state whose default plan contains the 5+5+1 extended pass that the n = 31 ... 33 plans
+    (BASELINE config 5) are made of; its oracle run needs 60 GiB of host memory and a few minutes."""
     import torch
 
     import oracle
@@ -182,6 +184,10 @@ def test_dense_full_oracle_at_the_bench_kernels(n, k):
     shapes = lambda p: {(q["kernel"], tuple(q["steps"])) for q in p.describe()["passes"]}
     if n == 28:
         assert shapes(bench) <= shapes(plan) | {("tma2x", (5, 4, 1))} and ("tma2x", (5, 4, 1)) in shapes(plan)
+    if n == 31:
+        big = qft.Plan(33, 33)  # config 5's plan: three passes of this shape
+        assert shapes(big) == {("tma2x", (5, 5, 1))} and ("tma2x", (5, 5, 1)) in shapes(plan)
+        big.close()
     bench.close()
     plan.execute(x)
     torch.cuda.synchronize()
@@ -207,9 +213,6 @@ def test_config5_n33_tones_exact_and_k16():
     n = 33
     fr, ph = qi.tone_params(n, 4, 5)
     x = torch.empty(1 << n, dtype=torch.complex64, device="cuda")
-    nchunks = 1 << (n - 22)
-    rng = np.random.default_rng(33)
-    near = sorted({int(f) >> 22 for f in fr})
     for k in (33, 16):
         qi.multi_tone_device(n, fr, ph, device="cuda", out=x)
         assert abs(lc.norm2(x) - 1.0) < 1e-5
@@ -223,12 +226,76 @@ def test_config5_n33_tones_exact_and_k16():
         assert abs(lc.norm2(x) - 1.0) < 1e-4
         got = x[torch.as_tensor(Ks, device="cuda")].to(torch.complex128)
         _check_samples(got, want, ("n = 33 tones", k))
-        chunks = sorted(set(near) | {int(c) for c in rng.integers(0, nchunks, size=40)})
-        rel, _, mx, rmax = lc.tones_parity(x, n, k, fr, ph, chunk_bits=22, index_chunks=chunks)
+        # every output index (the full streaming relative L2 against the closed form),
+        # in chunks of 2^24: a store that lands a zero on the wrong zero is invisible, a non-zero anywhere is not
+        rel, den, mx, rmax = lc.tones_parity(x, n, k, fr, ph, chunk_bits=24, index_chunks=None)
         assert rel <= TOL_LARGE and rel <= REG_L2 and mx <= MAXABS_FRAC * rmax, (k, rel, mx, rmax)
+        assert abs(den - 1.0) < 1e-9
         if k == 33:
             g5 = x[torch.as_tensor(fr, device="cuda")].to(torch.complex128).cpu().numpy()
             assert np.max(np.abs(g5 - np.exp(1j * ph) / math.sqrt(5))) < 1e-4
+
+
+def test_config5_n33_gaussian_parseval_and_sampled_sums():
+    """A dense input through config 5's kernel (three 5+5+1 extended passes): every sampled output depends on all 2^33
+    inputs and has modulus about 2^-16.5, not 0 as almost everywhere for the tones.  In place: one 64 GiB buffer."""
+    import torch
+
+    import large_checks as lc
+    import paper_2606_18981_b200 as qft
+
+    if _free_gib() < 70:
+        pytest.skip("needs 70 GiB of free device memory")
+    n = 33
+    x = torch.empty(1 << n, dtype=torch.complex64, device="cuda")
+    fr, _ = qi.tone_params(n, 4, 5)
+    Ks = _sample_indices(n, fr, 36)
+    for k in (33, 16):
+        qi.gaussian_device(n, 6, device="cuda", out=x)
+        assert abs(lc.norm2(x) - 1.0) < 1e-5
+        want = lc.sampled_outputs(x, Ks, k)  # direct fp64 sums over the actual fp32 input, BEFORE the transform
+        plan = qft.Plan(n, k)
+        assert {(q["kernel"], tuple(q["steps"])) for q in plan.describe()["passes"]} == {("tma2x", (5, 5, 1))}
+        plan.execute(x)
+        torch.cuda.synchronize()
+        plan.close()
+        assert abs(lc.norm2(x) - 1.0) < 1e-4
+        got = x[torch.as_tensor(Ks, device="cuda")].to(torch.complex128)
+        assert float(want.abs().min().item()) > 1e-8  # dense: no sampled output is (nearly) zero
+        _check_samples(got, want, ("n = 33 Gaussian", k))
+
+
+@pytest.mark.parametrize("k", [31, 9])
+def test_dense_n31_extended_plan_against_plain_plan(k):
+    """Every output element of a Gaussian input at n = 31, the default plan (5+5+1 extended passes through tensor
+    memory, as at n = 33) against the plan without the extension (QFT_FLAG_NO_EXT_TILE: four plain 2^14-tile passes
+    of the kind that the smaller sizes compare with the oracle element by element).  Two independent schedules and
+    kernel instantiations, no host oracle: 2 x 16 GiB on the device."""
+    import torch
+
+    import paper_2606_18981_b200 as qft
+
+    if _free_gib() < 40:
+        pytest.skip("needs 40 GiB of free device memory")
+    n = 31
+    x = qi.gaussian_device(n, 8, device="cuda")
+    y = x.clone()
+    ext = qft.Plan(n, k)
+    plain = qft.Plan(n, k, flags=qft.QFT_FLAG_NO_EXT_TILE)
+    shapes = lambda p: [(q["kernel"], tuple(q["steps"])) for q in p.describe()["passes"]]
+    assert ("tma2x", (5, 5, 1)) in shapes(ext) and all(kind == "tma2" for kind, _ in shapes(plain))
+    ext.execute(x)
+    plain.execute(y)
+    torch.cuda.synchronize()
+    ext.close()
+    plain.close()
+    cp = ChunkedParity()
+    C = 1 << 26
+    for c in range((1 << n) // C):
+        cp.add(x[c * C:(c + 1) * C], y[c * C:(c + 1) * C].to(torch.complex128))
+    rel, mx = cp.check(n, ("n = 31 extended vs plain", k))
+    assert abs(cp.den - 1.0) < 1e-4  # and the reference side is a unit vector (Parseval)
+    print(f"n=31 k={k} extended vs plain: rel_l2={rel:.3e} max_abs/max_ref={mx:.3e}")
 
 
 def test_max_size_n34_tones_exact():

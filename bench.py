@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--extrapolate-cpu", action="store_true",
                     help="also estimate the oracle's time at the bench n from a few gates (labelled as extrapolated)")
     ap.add_argument("--sweep", default="26,33", help="comma list of extra n to time briefly ('' = none)")
+    ap.add_argument("--sweep-fused", default="26:2,26:4,26:6",
+                    help="comma list of n:max_fused_qubits timed briefly (BASELINE config 3; '' = none)")
     ap.add_argument("--small-n", default="20,22", help="comma list of launch-bound sizes to time over 1000 back-to-back "
                                                        "transforms ('' = none)")
     ap.add_argument("--batched", default="12:16,16:12,22:6", help="comma list of n:log2_batch pairs to time briefly (batched "
@@ -151,12 +153,13 @@ def max_over_ranks(x: float, world: int, device) -> float:
     return float(t.item())
 
 
-def time_config(qft, torch, n, k, args, steps, warmup, per_pass=True, log2_batch=0):
+def time_config(qft, torch, n, k, args, steps, warmup, per_pass=True, log2_batch=0, max_fused=None):
     """Device-resident timing of qft_execute on a fresh synthetic state; returns a dict."""
     import qft_inputs as qi
 
     dev = torch.device("cuda", torch.cuda.current_device())
-    plan = qft.Plan(n, n if k is None else k, args.max_fused, -1, qft.QFT_NORM_UNITARY, args.tile_bits,
+    plan = qft.Plan(n, n if k is None else k, args.max_fused if max_fused is None else max_fused, -1,
+                    qft.QFT_NORM_UNITARY, args.tile_bits,
                     args.hub_bits, args.flags, log2_batch)
     n = n + log2_batch  # address bits of the state
     state = torch.empty(1 << n, dtype=torch.complex64, device=dev)
@@ -288,7 +291,11 @@ def run_reference(args):
         "impl": "reference", "metric": "dft_equiv_gflops", "value": gf, "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": t_step * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_text(n, args.k), "n_qubits": n,
+        "config": {"workload": workload_text(n, args.k) if n_eff == n else
+                   (workload_text(n, args.k) + f"; THIS ARM's steps are whole circuits at n={n_eff} "
+                    f"({8 * (1 << n_eff) / 2 ** 20:.0f} MiB states in complex64 terms, fp64 on the host): a bounded "
+                    f"sample of that workload, see cpu_baseline.sample"),
+                   "n_qubits": n,
                    "aqft_cutoff_k": n if args.k is None else min(args.k, n),
                    "implementation": "CPU oracle (gate-by-gate fp64, OpenMP)", "sample_n_qubits": n_eff},
         "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
@@ -487,6 +494,30 @@ def main():
             del r
             torch.cuda.empty_cache()
 
+    # ---- BASELINE config 3: the fused-window cap (the paper's max_fused_size) swept at n = 26 ----
+    fused_sweep = []
+    if args.sweep_fused and rank == 0 and world == 1:
+        try:
+            del state
+            plan.close()
+        except Exception:  # already released by the sweep
+            pass
+        torch.cuda.empty_cache()
+        for pair in [v for v in args.sweep_fused.split(",") if v]:
+            fn, fw = (int(v) for v in pair.split(":"))
+            r = time_config(qft, torch, fn, None, args, 10, 3, per_pass=True, max_fused=fw)
+            slow = max(r["pass_ms"])
+            gbs = r["passes"] * 16.0 * (1 << fn) / (r["median_ms"] * 1e-3) / 1e9
+            fused_sweep.append({"n": fn, "max_fused_qubits": fw, "passes": r["passes"], "steps": 10,
+                                "median_ms": r["median_ms"],
+                                "gflops": 5.0 * (1 << fn) * fn / (r["median_ms"] * 1e-3) / 1e9,
+                                "gbs": gbs, "roofline_frac": gbs / peak,
+                                "slowest_pass_frac": 16.0 * (1 << fn) / (slow * 1e-3) / 1e9 / peak,
+                                "pass_kernels": sorted({p["kernel"] for p in r["plan"].describe()["passes"]})})
+            r["plan"].close()
+            del r
+            torch.cuda.empty_cache()
+
     batched = []
     if args.batched and rank == 0 and world == 1:
         try:
@@ -578,8 +609,11 @@ def main():
         }
         if variants:
             line["variants"] = variants
+        line["tensor_map_fallbacks"] = qft.qft_tensor_map_fallbacks()  # launches that took the slow generic path: 0
         if sweep:
             line["sweep"] = sweep
+        if fused_sweep:
+            line["max_fused_sweep"] = fused_sweep
         if batched:
             line["batched"] = batched
         if small:

@@ -234,7 +234,8 @@ qft_status_t qft_plan_describe(qft_plan_t plan, char* buf, size_t len);
  *   qft_num_qubits_for   n = max(1, ceil(log2 length)) of PAPER.md:124 ("we choose n = ceil(log2 N) qubits and
  *                 allocate a 2^n-element state vector"); -1 if length is 0 or exceeds 2^34.
  *   qft_encode_padded    the whole input-encoding step of PAPER.md:124 for an array of any length <= 2^n_qubits:
- *                 copies device_x (float2[length], device memory; may be device_state itself) to the front of
+ *                 copies device_x (float2[length], device memory; device_state itself or a buffer disjoint from
+ *                 it, QFT_ERR_INVALID_ARG for a partial overlap) to the front of
  *                 device_state (float2[2^n_qubits]), zero-fills the rest, then qft_encode.  Note that the
  *                 transform of the padded state is the 2^n-point DFT of the padded array, not a length-point DFT.
  * The reductions keep one 32-byte scratch buffer per device (allocated at the first call on that device) and
@@ -291,6 +292,14 @@ const char* qft_static_last_error(void);
  * tile when applied, that tiles are closed under the store permutation, and
  * that every qubit ends on its bit-reversed address.  QFT_OK or QFT_ERR_INTERNAL. */
 qft_status_t qft_plan_self_check(qft_plan_t plan);
+
+/*
+ * qft_tensor_map_fallbacks -- how many pass launches of this process (any plan, any thread) ran the generic
+ * shared-memory kernel because the driver refused to encode the pass's tensor map.  qft_execute still returns QFT_OK
+ * then and the result is the same, but such a pass runs at roughly a tenth of the TMA kernel's bandwidth; the driver
+ * accepts every map the planner produces today, so anything but 0 deserves a look.  bench.py reports it.
+ */
+unsigned long long qft_tensor_map_fallbacks(void);
 
 const char* qft_status_string(qft_status_t status);
 /* Last CUDA error text seen by this library on the calling thread ("" if none). */

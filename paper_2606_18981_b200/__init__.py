@@ -32,7 +32,7 @@ EXPORTS = [
     "qft_plan_self_check", "qft_status_string", "qft_last_cuda_error",
     "qft_plan_shard_info", "qft_plan_shard_check", "qft_execute_pass_shard",
     "qft_norm_sq", "qft_encode", "qft_rescale", "qft_fidelity", "qft_leakage",
-    "qft_fidelity_batched_static", "qft_static_last_error",
+    "qft_fidelity_batched_static", "qft_static_last_error", "qft_tensor_map_fallbacks",
 ]
 
 _lib = None
@@ -118,6 +118,8 @@ def load() -> ctypes.CDLL:
     L.qft_last_cuda_error.restype = ctypes.c_char_p
     L.qft_fidelity_batched_static.argtypes = [vp, vp, ci, ci, vp, vp]
     L.qft_fidelity_batched_static.restype = ci
+    L.qft_tensor_map_fallbacks.argtypes = []
+    L.qft_tensor_map_fallbacks.restype = ctypes.c_ulonglong
     L.qft_static_last_error.argtypes = []
     L.qft_static_last_error.restype = ctypes.c_char_p
     _lib = L
@@ -304,6 +306,11 @@ def qft_fidelity(device_a_ptr: int, device_b_ptr: int, n_qubits: int, stream: in
 
 def qft_leakage(device_state_ptr: int, n_qubits: int, bin_index: int, stream: int = 0) -> float:
     return _dbl_call("qft_leakage", device_state_ptr, n_qubits, int(bin_index), stream)
+
+
+def qft_tensor_map_fallbacks() -> int:
+    """Pass launches of this process that fell back to the generic kernel (tensor map refused); 0 is the expected value."""
+    return int(load().qft_tensor_map_fallbacks())
 
 
 def qft_static_last_error() -> str:

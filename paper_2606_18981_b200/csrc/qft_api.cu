@@ -278,6 +278,8 @@ const char* qft_status_string(qft_status_t status) {
 
 const char* qft_last_cuda_error(void) { return g_cuda_err.c_str(); }
 
+unsigned long long qft_tensor_map_fallbacks(void) { return qft_launch_map_fallbacks(); }
+
 #ifdef QFT_PHASE_TIMING
 // profiling builds only: device buffer of 16 counters the TMA kernel of pass `pass_index` accumulates into
 int qft_debug_set_phase_buffer(qft_plan_t plan, int pass_index, void* device_counters) {

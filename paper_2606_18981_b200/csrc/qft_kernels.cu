@@ -19,6 +19,7 @@
 #include "qft_launch.h"
 
 #include <algorithm>
+#include <atomic>
 
 namespace qftk {
 
@@ -341,6 +342,11 @@ static bool get_map(const QftPassDesc& d, QftPassCache* cache, int dev, void* sr
     return true;
 }
 
+// Launches that ran the generic kernel because the driver refused the pass's tensor map (about 10x slower, same
+// result): counted so that the slow path cannot be taken unnoticed (qft_tensor_map_fallbacks, include/qft.h).
+static std::atomic<unsigned long long> g_map_fallbacks{0};
+unsigned long long qft_launch_map_fallbacks() { return g_map_fallbacks.load(std::memory_order_relaxed); }
+
 static int tma2_ctas_per_sm(const QftPassDesc& d, size_t smem) {
     int per_sm = d.f == 13 ? 2 : (d.f == 12 ? 4 : 1);
     while (per_sm > 1 && per_sm * (smem + 1024) > 227 * 1024) --per_sm;
@@ -365,6 +371,7 @@ static cudaError_t launch_tma2(const QftPassDesc& d_in, QftPassCache* cache, int
             QftPassDesc g = d;
             g.kernel = QFT_KERNEL_GENERIC;
             g.log2_threads = 8;
+            g_map_fallbacks.fetch_add(1, std::memory_order_relaxed);
             // A cold path: a fresh cache per launch, so the shared-memory attribute is set (idempotent) for whichever
             // generic instantiation this pass picks; one shared cache would skip it for the second instantiation.
             QftPassCache plain;

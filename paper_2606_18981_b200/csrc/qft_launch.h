@@ -25,3 +25,5 @@ struct QftPassCache {
 // different one only if qft_pass_reads_through_tensor_map(d), else cudaErrorNotSupported).
 cudaError_t qft_launch_pass(const QftPassDesc& d, QftPassCache* cache, void* src, void* state, cudaStream_t stream);
 bool qft_pass_reads_through_tensor_map(const QftPassDesc& d);
+// Pass launches so far (this process, any plan) that fell back to the generic kernel because no tensor map was granted.
+unsigned long long qft_launch_map_fallbacks();

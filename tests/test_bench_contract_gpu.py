@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 def test_bench_line_has_the_contract_keys():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--n", "22", "--steps", "5", "--warmup", "3",
-                        "--batched", "10:12", "--sweep", "24"], capture_output=True, text=True, timeout=900)
+                        "--batched", "10:12", "--sweep", "24", "--sweep-fused", "22:2,22:6"], capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [ln for ln in r.stdout.splitlines() if ln.strip()]
     assert len(lines) == 1
@@ -36,5 +36,8 @@ def test_bench_line_has_the_contract_keys():
     assert d["batched"][0]["n"] == 10 and d["batched"][0]["log2_batch"] == 12
     sw = d["sweep"][0]
     assert sw["n"] == 24 and sw["passes"] >= sw["ideal_passes"] and 0 < sw["roofline_frac"] < 1.2
+    fs = d["max_fused_sweep"]  # BASELINE config 3's dimension (max_fused_size)
+    assert [(f["n"], f["max_fused_qubits"]) for f in fs] == [(22, 2), (22, 6)] and fs[0]["passes"] > fs[1]["passes"] >= 3
+    assert all(0 < f["slowest_pass_frac"] <= f["roofline_frac"] * 1.5 and f["median_ms"] > 0 for f in fs)
     assert "seconds_n22" in cb and "seconds_n26" in cb and len(cb["trials_n26"]) == 3  # whole circuits, timed
     assert rf["traffic"] is None or rf["traffic_source"]

@@ -387,15 +387,15 @@ def main():
     bytes_per_launch = 16.0 * N  # 8 B read + 8 B written per amplitude per pass
     achieved = bytes_per_launch / (dom_ms * 1e-3) / 1e9
     # measured DRAM bytes per launch of the dominant kernel: a COPY of the figure in the committed ncu --set full
-    # capture (profiles/r02_traffic.csv: n, kernel, bytes), null when that file has no row for this (n, kernel)
+    # capture (profiles/r03_traffic.csv: n, kernel, bytes), null when that file has no row for this (n, kernel)
     traffic, traffic_source = None, None
     try:
-        with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r03_traffic.csv")) as fh:
             for row in fh:
                 f = [v.strip() for v in row.split(",")]
                 if len(f) >= 3 and f[0] == str(n) and f[1] == dom:
                     traffic = float(f[2])
-                    traffic_source = ("profiles/r02_traffic.csv (dram__bytes_read.sum + dram__bytes_write.sum of one "
+                    traffic_source = ("profiles/r03_traffic.csv (dram__bytes_read.sum + dram__bytes_write.sum of one "
                                       "ncu --set full capture of this kernel at this n; not re-measured in this run)")
     except Exception:
         pass

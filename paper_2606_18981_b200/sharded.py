@@ -12,9 +12,11 @@ A pass whose tiles hold no rank bit touches only the rank's own shard; a pass wh
 writes its peers' shards directly from the kernel (TMA loads, plain stores): the exchange is fused into the pass, there
 is no collective on the data path.  The barrier is whatever the caller passes (torch.distributed.barrier with NCCL).
 
-Tested on this round's single GPU only in the degenerate form `LocalShards` (all shards on one device, the ranks' shares
-enqueued one after the other: tests/test_sharded.py) plus the file-descriptor exchange between processes on the CPU;
-NOT run on more than one GPU.  PyTorch is not needed here; the driver API comes from cuda-python.
+Tested on a single GPU only: `LocalShards` (all shards on one device, the ranks' shares enqueued one after the other),
+the file-descriptor exchange between processes on the CPU, and `ShardedQft` itself as 1, 2 and 4 processes that all use
+the one GPU (each creates, exports, imports and maps real shards and runs its share of every pass between barriers:
+tests/test_sharded.py).  NOT run on more than one GPU: nothing here has seen a peer mapping over NVLink, and no time was
+taken.  PyTorch is not needed here; the driver API comes from cuda-python.
 """
 from __future__ import annotations
 
